@@ -85,10 +85,10 @@ inline bool lu_factor(double* A, int* piv, int N) {
   return true;
 }
 inline void lu_solve(const double* A, const int* piv, int N, double* b) {
-  for (int k = 0; k < N; ++k) {
-    std::swap(b[k], b[piv[k]]);
+  // P A = L U with whole rows swapped in lu_factor, so L belongs to the FINAL row order: apply all of P first
+  for (int k = 0; k < N; ++k) std::swap(b[k], b[piv[k]]);
+  for (int k = 0; k < N; ++k)
     for (int i = k + 1; i < N; ++i) b[i] -= A[i * N + k] * b[k];
-  }
   for (int k = N - 1; k >= 0; --k) {
     b[k] /= A[k * N + k];
     for (int i = 0; i < k; ++i) b[i] -= A[i * N + k] * b[k];
@@ -121,6 +121,7 @@ struct Problem {
   virtual int dim() const = 0;
   virtual void f(const double* y, double* out) const = 0;
   virtual void jac(const double* y, const double* f0, double h, double* J) const = 0;
+  virtual int jac_rhs_evals() const { return 0; }  // RHS evaluations one jac() call costs (N for FD)
   virtual ~Problem() {}
 };
 
@@ -132,6 +133,7 @@ struct Reactor : Problem {
   void jac(const double* y, const double* f0, double h, double* J) const override {
     if (jac_mode == 0) jac_complex_step(m, y, p, J); else jac_fd(m, y, p, f0, h, rtol, atol, J);
   }
+  int jac_rhs_evals() const override { return jac_mode == 0 ? 0 : m.K + 1; }
 };
 
 // ---- ROS4 attempt (O4): Eq. 6-7 ------------------------------------------------------------------
@@ -142,7 +144,7 @@ inline bool ros4_step(const Problem& pr, const double* y, double h, double* ynew
   std::vector<double> f0(N), J(N * N), A(N * N), u1(N), u2(N), u3(N), u4(N), yt(N), ft(N);
   std::vector<int> piv(N);
   pr.f(y, f0.data()); c.rhs++;
-  pr.jac(y, f0.data(), h, J.data()); c.jac++;
+  pr.jac(y, f0.data(), h, J.data()); c.jac++; c.rhs += pr.jac_rhs_evals();
   for (int i = 0; i < N; ++i)
     for (int j = 0; j < N; ++j) A[i * N + j] = (i == j ? 1.0 / (h * gam) : 0.0) - J[i * N + j];
   c.lu++;
