@@ -1,0 +1,288 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement (BASELINE.json): RHS evaluations/s (FP64) on config 2, the 53-species /
+325-reaction synthetic mechanism over 1,048,576 reactor states, plus reactors/s of the integrators (extra keys).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--extras 0|1]
+
+A "step" is one pass of the hot path over the whole batch: one ck_rhs call on all n states (device-resident
+inputs; 914 MB touched per pass, larger than the 126 MB L2, so no L2 flush is needed between steps).
+Multi-GPU (torchrun): reactors are independent, every rank evaluates its own n states (weak scaling, no
+collective on the data path); value = total states / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+WORKLOAD = "C2: RHS-only, synthetic 53-species/325-reaction mechanism, 1,048,576 states, FP64"
+METRIC = "rhs_evals_per_s"
+UNIT = "RHS evals/s"
+# FP64 vector peak derived from unit counts and clocks:
+# 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
+PEAK_SLOTS = 148 * 64 * 1.965e9
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index=0, period=0.05):
+        self.index, self.period = index, period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+
+    def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+            return self
+        self._thr = threading.Thread(target=self._run, daemon=True)
+        self._thr.start()
+        return self
+
+    def _run(self):
+        nv = self._nv
+        names = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def time_oracle_rhs(mech, y, p, target_s=12.0):
+    """Oracle RHS on a bounded sample of the workload, all host cores (omp dynamic over states)."""
+    from oracle import ck_oracle
+    O = ck_oracle.Mech(mech)
+    cores = min(oracle_cores(), ck_oracle.max_threads())
+    ns = 4096
+    t0 = time.perf_counter(); O.rhs(y[:, :ns].copy(), p[:ns].copy(), nthreads=cores); t1 = time.perf_counter()
+    rate = ns / (t1 - t0)
+    ns = int(min(y.shape[1], max(ns, rate * target_s)))
+    ys = np.ascontiguousarray(y[:, :ns]); ps = np.ascontiguousarray(p[:ns])
+    t0 = time.perf_counter(); O.rhs(ys, ps, nthreads=cores); t1 = time.perf_counter()
+    return ns / (t1 - t0), cores, ns, t1 - t0
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from synth_inputs import make_config
+    mech, y, p, _ = make_config("C2", n=65536)
+    per_step = max(1.0, 60.0 / max(1, args.steps + args.warmup))
+    vals = []
+    for i in range(args.warmup + args.steps):
+        v, cores, ns, dt = time_oracle_rhs(mech, y, p, target_s=min(per_step, 10.0))
+        if i >= args.warmup:
+            vals.append((v, dt))
+    value = float(np.mean([v for v, _ in vals]))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([d for _, d in vals])), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "sample": f"{ns} states per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{ns} of 1,048,576 states per step, omp dynamic over states"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def integrator_extras(torch, ck, dev):
+    """Reactors/s of the integrators on configs 3-5 (device-resident inputs), best of 2 after one warm-up.
+    Returns {} entries with an "error" key while an integrator is not available."""
+    from synth_inputs import make_config
+    out = {}
+    for name in ("C1", "C3", "C4", "C5"):
+        try:
+            mech, y, p, cfg = make_config(name)
+            M = ck.Mechanism(mech, device=dev.index or 0)
+            y0 = torch.from_numpy(y).to(dev); pd = torch.from_numpy(p).to(dev)
+            best, res = None, None
+            ws = None
+            for it in range(3):
+                yy = y0.clone()
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize(); e0.record()
+                res = M.integrate(cfg["call"], yy, pd, cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"], ws=ws)
+                e1.record(); torch.cuda.synchronize()
+                ws = res["ws"]
+                ms = e0.elapsed_time(e1)
+                if it >= 1:
+                    best = ms if best is None else min(best, ms)
+            rep = res["report"]
+            slots_rhs = M.rhs_slots()
+            out[name] = {"call": cfg["call"], "n": int(y.shape[1]), "ms": best, "reactors_per_s": y.shape[1] / (best * 1e-3),
+                         "rhs_evals_per_s": rep["rhs_evals"] / (best * 1e-3), "attempts": rep["attempts"],
+                         "accepted": rep["accepted"], "rejected": rep["rejected"], "rounds": rep["rounds"],
+                         "simt_efficiency": rep["simt_efficiency"], "waste_p32_static": rep["waste_p32"],
+                         "n_failed": rep["n_failed"],
+                         "rhs_only_roofline_frac": rep["rhs_evals"] * slots_rhs / (best * 1e-3) / PEAK_SLOTS}
+            M.close()
+        except Exception as ex:  # integrator not available yet / failed: report, do not hide
+            out[name] = {"error": str(ex)[:200]}
+    return out
+
+
+def run_ours(args):
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    mech, y, p, cfg = make_config("C2")          # every rank: its own n states (seed offset by rank)
+    if rank:
+        rng = np.random.default_rng(1000 + rank)
+        perm = rng.permutation(y.shape[1]); y = np.ascontiguousarray(y[:, perm]); p = np.ascontiguousarray(p[perm])
+    n = y.shape[1]
+    M = ck.Mechanism(mech, device=local)
+    yd = torch.from_numpy(y).to(dev); pd = torch.from_numpy(p).to(dev)
+    out = torch.empty_like(yd)
+    slots = M.rhs_slots()
+    alg_bytes = (2 * M.K + 3) * 8 * n
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        M.rhs(yd, pd, out=out)
+    barrier()
+    clocks = ClockSampler(local).start()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    ev[0].record()
+    for i in range(args.steps):
+        M.rhs(yd, pd, out=out)
+        ev[i + 1].record()
+    barrier()
+    clk = clocks.stop()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per_launch_ms = float(np.mean([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]))
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); total_ms = float(t.item())
+    value = world * n * args.steps / (total_ms * 1e-3)
+
+    # end to end through the host-pointer C-ABI call: pinned host buffers, H2D + kernel + D2H per step
+    yh = torch.from_numpy(y).pin_memory(); ph = torch.from_numpy(p).pin_memory(); oh = torch.empty_like(yh).pin_memory()
+    ynp, pnp, onp = yh.numpy(), ph.numpy(), oh.numpy()
+    e2e_steps = max(2, min(args.steps, 5))
+    M.rhs_host(ynp, pnp, out=onp)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        M.rhs_host(ynp, pnp, out=onp)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e = {"value": world * n * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(ynp.nbytes + pnp.nbytes),
+           "d2h_bytes_per_step": int(onp.nbytes), "steps": e2e_steps}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    achieved = slots * n / (per_launch_ms * 1e-3)
+    measured_peak = None
+    try:
+        measured_peak = ck.fp64_peak(local)
+    except Exception:
+        pass
+    traffic = None
+    tf = os.path.join(ROOT, "profiles", "rhs_kernel_traffic.json")
+    if os.path.exists(tf):
+        try:
+            traffic = json.load(open(tf)).get("dram_bytes_per_launch")
+        except Exception:
+            pass
+    roofline = {"bound": "alu", "kernel": "ck::rhs_kernel", "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
+                "unit": "TFLOP/s", "frac": achieved / PEAK_SLOTS, "traffic": traffic,
+                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
+                "slots_per_eval": slots, "fp64_pipe_inst_per_s": achieved,
+                "measured_dfma_peak_inst_per_s": measured_peak,
+                "frac_of_measured_dfma_peak": (achieved / measured_peak) if measured_peak else None,
+                "hbm_alg_bytes_per_launch": alg_bytes, "hbm_achieved_GBs": alg_bytes / (per_launch_ms * 1e-3) / 1e9,
+                "hbm_frac_of_measured": alg_bytes / (per_launch_ms * 1e-3) / 1e9 / 6554.2}
+    cpu_v, cores, ns, cpu_dt = time_oracle_rhs(mech, y, p)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "n_states_per_gpu": n, "l2": "inputs (914 MB per pass) larger than L2; no flush",
+                       "parallelism": f"independent reactors x{world}"},
+            "clocks": clk, "e2e": e2e, "gpu_launches": args.steps,
+            "roofline": roofline,
+            "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{ns} of {n} states, one pass, {cpu_dt:.1f} s, omp dynamic over states"}}
+    if args.extras:
+        line["integrators"] = integrator_extras(torch, ck, dev)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--extras", type=int, default=1, help="also time the integrators on configs 1,3,4,5 (rank 0, N=1)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if int(os.environ.get("WORLD_SIZE", "1")) > 1:
+            args.extras = 0
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,72 @@
+// Internal declarations shared by the libck translation units (product path; no oracle code).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/ck.h"
+
+namespace ck {
+
+constexpr double R_U = 8.31446261815324e7;  // erg/(mol K)
+constexpr double R_CAL = 1.98720425864083;  // cal/(mol K)
+constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere")
+constexpr int MAX_TINT = 8;                 // temperature intervals (distinct t_mid values + 1)
+
+// Device view of the packed mechanism (all pointers into one device arena; passed by value to kernels).
+// Reactions are regrouped by type: [0,r_tb) plain, [r_tb,r_lind) three-body, [r_lind,r_troe) Lindemann,
+// [r_troe,R) Troe.  Every per-reaction array is SoA over the regrouped index.
+struct MechDev {
+  int K, R, nT, Kpad;
+  int r_tb, r_lind, r_troe;
+  double tedge[MAX_TINT];     // interval t holds tedge[t-1] < T <= tedge[t]; nT-1 finite edges
+  const double* W;            // [K]
+  const double* invW;         // [K]
+  const double* nlo;          // [7][K] NASA-7, T <= t_mid
+  const double* nhi;          // [7][K]
+  const double* tmid;         // [K]
+  const double* lnA;          // [R]  Eq. 15: ln k_f = lnA + beta lnT - Ta/T
+  const double* beta;         // [R]
+  const double* Ta;           // [R]  Ea / R_cal
+  const double* krc;          // [nT][7][R]  ln k_r = c0 + c1 lnT + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4
+  const int* part;            // [6][R]  slots 0-2 reactants, 3-5 products: (species << 8) | nu ; 0 = empty
+  const int* eptr;            // [R - r_tb + 1] CSR of non-unit efficiencies, rows = reactions r_tb..R-1
+  const int* espec;
+  const double* eval1;        // alpha - 1
+  const double* lnA0;         // [R - r_lind] low-pressure limit of falloff rows
+  const double* beta0;
+  const double* Ta0;
+  const double* troe;         // [4][R - r_troe]  a, 1/T***, 1/T*, T** (T** < 0: absent)
+  // transposed stoichiometry (gather form for cooperative kernels): species k <- sum nu_ki q_i
+  const int* tptr;            // [K+1]
+  const int* tent;            // (reaction << 8) | (net nu + 128)
+  const int* perm;            // [R] regrouped index -> caller's reaction index
+};
+
+void set_error(const char* fmt, ...);
+int32_t cuda_fail(cudaError_t e, const char* what);
+
+}  // namespace ck
+
+struct ck_mech {
+  int device = 0;
+  ck::MechDev dev;            // device view
+  void* arena = nullptr;      // device allocation backing `dev`
+  size_t arena_bytes = 0;
+  // host copies used by the launch logic / roofline accounting
+  int K = 0, R = 0;
+  int n_tb = 0, n_lind = 0, n_troe = 0, n_rev = 0;
+  long long n_part = 0, n_eff = 0;
+  // cached device staging buffers of the *_host entry points
+  void* stage = nullptr;
+  size_t stage_bytes = 0;
+  cudaStream_t hstream = nullptr;
+};
+
+#define CK_CUDA(call)                                                    \
+  do {                                                                   \
+    cudaError_t e_ = (call);                                             \
+    if (e_ != cudaSuccess) return ck::cuda_fail(e_, #call);              \
+  } while (0)
