@@ -44,10 +44,75 @@ __device__ __forceinline__ double thermo_dcp(const MechDev& m, int k, const TSta
   return fma(fma(fma(4.0 * a5, T, 3.0 * a4), T, 2.0 * a3), T, a2);
 }
 
-__device__ __forceinline__ double ipow_small(double x, int n) {
-  double r = x;
-  for (int i = 1; i < n; ++i) r *= x;
-  return r;
+// exp(x) for the rate constants: x = n ln2 + r, |r| <= ln2/2, degree-11 polynomial in Estrin form (short
+// dependency chains: the kernels are latency-, not throughput-limited on this function), 2^n applied to
+// the exponent field.  Coefficients: Chebyshev-node interpolation of e^r on [-ln2/2, ln2/2] (max relative
+// error 1.6e-17 before rounding).  x < -708 returns 0 (so c0 = -inf encodes an irreversible reaction),
+// x > 709 returns +inf.
+__device__ __forceinline__ double ck_exp(double x) {
+  const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52
+  const double t = fma(x, 1.4426950408889634074, MAGIC);
+  const int n = __double2loint(t);
+  const double nf = t - MAGIC;
+  double r = fma(nf, -6.93147180369123816490e-01, x);
+  r = fma(nf, -1.90821492927058770002e-10, r);
+  const double r2 = r * r;
+  const double p01 = 1.0 + r;
+  const double p23 = fma(0x1.555555555555ap-3, r, 0x1.0000000000011p-1);
+  const double p45 = fma(0x1.111111110f21ep-7, r, 0x1.555555554f0bap-5);
+  const double p67 = fma(0x1.a01a01b1461c5p-13, r, 0x1.6c16c1880029fp-10);
+  const double p89 = fma(0x1.71ddf56d8deb5p-19, r, 0x1.a01991a10d9aep-16);
+  const double pab = fma(0x1.af632a0f7e2cep-26, r, 0x1.28b4101c77212p-22);
+  const double r4 = r2 * r2;
+  const double q0 = fma(p23, r2, p01);
+  const double q1 = fma(p67, r2, p45);
+  const double q2 = fma(pab, r2, p89);
+  const double r8 = r4 * r4;
+  const double s0 = fma(q1, r4, q0);
+  double res = fma(q2, r8, s0);
+  res = __hiloint2double(__double2hiint(res) + (n << 20), __double2loint(res));
+  res = (x < -708.0) ? 0.0 : res;
+  res = !(x <= 709.0) ? x + __longlong_as_double(0x7ff0000000000000LL) : res;  // overflow -> inf, NaN -> NaN
+  return res;
+}
+
+// Constants of one reaction gathered into registers (from the SoA arrays or from a staged rpack row).
+struct RxnConst {
+  double lnA, beta, Ta, c0, c1, c2, c3, c4, c5, c6;
+  int slot[6];  // species index (or the dummy K) of the three reactant and three product slots
+};
+__device__ __forceinline__ RxnConst load_rxn_global(const MechDev& m, int r, int tint) {
+  RxnConst k;
+  const int R = m.R;
+  k.lnA = __ldg(m.lnA + r); k.beta = __ldg(m.beta + r); k.Ta = __ldg(m.Ta + r);
+  const double* c = m.krc + (size_t)tint * 7 * R + r;
+  k.c0 = __ldg(c); k.c1 = __ldg(c + R); k.c2 = __ldg(c + 2 * (size_t)R); k.c3 = __ldg(c + 3 * (size_t)R);
+  k.c4 = __ldg(c + 4 * (size_t)R); k.c5 = __ldg(c + 5 * (size_t)R); k.c6 = __ldg(c + 6 * (size_t)R);
+#pragma unroll
+  for (int s = 0; s < 6; ++s) k.slot[s] = __ldg(m.slot + (size_t)s * R + r);
+  return k;
+}
+// row = pointer to the reaction's rpack row (shared or global memory, 16-byte aligned)
+__device__ __forceinline__ RxnConst load_rxn_row(const double* row, int tint) {
+  RxnConst k;
+  const double2 a = *reinterpret_cast<const double2*>(row);
+  const double2 b = *reinterpret_cast<const double2*>(row + 2);
+  k.lnA = a.x; k.beta = a.y; k.Ta = b.x;
+  const unsigned lo = (unsigned)__double2loint(b.y), hi = (unsigned)__double2hiint(b.y);
+  k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
+  k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  const double2* c = reinterpret_cast<const double2*>(row + 4 + 8 * tint);
+  const double2 c01 = c[0], c23 = c[1], c45 = c[2], c67 = c[3];
+  k.c0 = c01.x; k.c1 = c01.y; k.c2 = c23.x; k.c3 = c23.y; k.c4 = c45.x; k.c5 = c45.y; k.c6 = c67.x;
+  return k;
+}
+
+// Rate constants of Eq. 15 and of Eq. 16-18 folded into one polynomial (ck_mech.cu)
+__device__ __forceinline__ void rate_constants(const RxnConst& k, const TState& t, double& kf, double& kr) {
+  kf = ck_exp(fma(k.beta, t.lnT, k.lnA) - k.Ta * t.invT);
+  const double T = t.T;
+  const double poly = fma(fma(fma(k.c6, T, k.c5), T, k.c4), T, k.c3) * T;
+  kr = ck_exp(fma(k.c1, t.lnT, k.c0) + fma(k.c2, t.invT, poly));
 }
 
 // Everything the Jacobian needs about one reaction besides q itself.
@@ -60,17 +125,14 @@ struct RateAux {
 
 // Rate of progress q_i of regrouped reaction r.  WANT_AUX also fills the derivative pieces.
 template <int CS, bool WANT_AUX>
-__device__ __forceinline__ double reaction_q(const MechDev& m, int r, const TState& t, const double* __restrict__ C,
-                                             double Ctot, RateAux* aux) {
+__device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnConst& k, const TState& t,
+                                             const double* __restrict__ C, double Ctot, RateAux* aux) {
   const int R = m.R;
-  const double beta = __ldg(m.beta + r), Ta = __ldg(m.Ta + r);
-  const double kf = exp(fma(beta, t.lnT, __ldg(m.lnA + r)) - Ta * t.invT);  // Eq. 15
-  const double* c = m.krc + (size_t)t.tint * 7 * R + r;
-  const double c1 = __ldg(c + R), c2 = __ldg(c + 2 * (size_t)R), c3 = __ldg(c + 3 * (size_t)R),
-               c4 = __ldg(c + 4 * (size_t)R), c5 = __ldg(c + 5 * (size_t)R), c6 = __ldg(c + 6 * (size_t)R);
+  const double beta = k.beta, Ta = k.Ta;
+  const double c1 = k.c1, c2 = k.c2, c3 = k.c3, c4 = k.c4, c5 = k.c5, c6 = k.c6;
   const double T = t.T;
-  const double poly = fma(fma(fma(c6, T, c5), T, c4), T, c3) * T;
-  const double kr = exp(fma(c1, t.lnT, __ldg(c)) + fma(c2, t.invT, poly));  // Eq. 16-18 folded (ck_mech.cu)
+  double kf, kr;
+  rate_constants(k, t, kf, kr);
   double ci = 1.0, dci_dM = 0.0, dci_dT = 0.0;
   if (r >= m.r_tb) {  // third-body / falloff factor c_i (reading G9)
     const int j = r - m.r_tb;
@@ -83,7 +145,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const TSta
     } else {
       const int jl = r - m.r_lind;
       const double beta0 = __ldg(m.beta0 + jl), Ta0 = __ldg(m.Ta0 + jl);
-      const double k0 = exp(fma(beta0, t.lnT, __ldg(m.lnA0 + jl)) - Ta0 * t.invT);
+      const double k0 = ck_exp(fma(beta0, t.lnT, __ldg(m.lnA0 + jl)) - Ta0 * t.invT);
       const double k0_kf = k0 / kf;
       const double Pr = k0_kf * M;
       const double inv1p = 1.0 / (1.0 + Pr);
@@ -93,10 +155,10 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const TSta
         const int jt = r - m.r_troe, nt = R - m.r_troe;
         const double a = __ldg(m.troe + jt), i3 = __ldg(m.troe + nt + jt), i1 = __ldg(m.troe + 2 * nt + jt),
                      T2 = __ldg(m.troe + 3 * nt + jt);
-        const double e3 = exp(-T * i3), e1 = exp(-T * i1);
+        const double e3 = ck_exp(-T * i3), e1 = ck_exp(-T * i1);
         double Fc = fma(1.0 - a, e3, a * e1);
         double e2 = 0.0;
-        if (T2 >= 0.0) { e2 = exp(-T2 * t.invT); Fc += e2; }
+        if (T2 >= 0.0) { e2 = ck_exp(-T2 * t.invT); Fc += e2; }
         const double il10 = 0.43429448190325182765;  // 1/ln 10
         const double ln10 = 2.30258509299404568402;
         const double Fcg = fmax(Fc, 1e-300), Prg = fmax(Pr, 1e-300);
@@ -106,7 +168,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const TSta
         const double den = fma(-0.14, x, nn);
         const double f1 = x / den;
         const double g = 1.0 / fma(f1, f1, 1.0);
-        F = exp(ln10 * lF * g);
+        F = ck_exp(ln10 * lF * g);
         if (WANT_AUX) {
           // ln F = ln10 * lF / (1 + f1^2);  f1 = x/den, x = lP + cc(lF), den = nn(lF) - 0.14 x
           const double df1_dx = nn / (den * den);              // (den + 0.14 x)/den^2 = nn/den^2
@@ -133,17 +195,9 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const TSta
       }
     }
   }
-  double pf = 1.0, pr = 1.0;  // Eq. 14, integer nu by repeated multiplication
-#pragma unroll
-  for (int s = 0; s < 3; ++s) {
-    const int e = __ldg(m.part + (size_t)s * R + r);
-    if (e) pf *= ipow_small(C[(size_t)(e >> 8) * CS], e & 255);
-  }
-#pragma unroll
-  for (int s = 3; s < 6; ++s) {
-    const int e = __ldg(m.part + (size_t)s * R + r);
-    if (e) pr *= ipow_small(C[(size_t)(e >> 8) * CS], e & 255);
-  }
+  // Eq. 14: products over the slots (nu copies of each species; the dummy slot holds C = 1)
+  const double pf = C[(size_t)k.slot[0] * CS] * C[(size_t)k.slot[1] * CS] * C[(size_t)k.slot[2] * CS];
+  const double pr = C[(size_t)k.slot[3] * CS] * C[(size_t)k.slot[4] * CS] * C[(size_t)k.slot[5] * CS];
   if (WANT_AUX) {
     aux->kf = kf; aux->kr = kr; aux->ci = ci; aux->pf = pf; aux->pr = pr;
     aux->dlnkf_dT = (beta + Ta * t.invT) * t.invT;

@@ -16,22 +16,30 @@ constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere", PAPER
 constexpr int MAX_TINT = 8;                 // temperature intervals (distinct t_mid values + 1)
 
 // Device view of the packed mechanism (all pointers into one device arena; passed by value to kernels).
-// Reactions are regrouped by type: [0,r_tb) plain, [r_tb,r_lind) three-body, [r_lind,r_troe) Lindemann,
+// Reactions are regrouped by type: [0,r_dup) plain with six distinct slot species, [r_dup,r_tb) plain with a
+// repeated species (nu >= 2 or a species on both sides), [r_tb,r_lind) three-body, [r_lind,r_troe) Lindemann,
 // [r_troe,R) Troe.  Every per-reaction array is SoA over the regrouped index.
+// Stoichiometry is stored as SLOTS: each side of a reaction is expanded to exactly three species indices,
+// nu copies of each participant, padded with the dummy index K (the kernels keep C[K] = 1 and a sink
+// accumulator at K), so rate products and the omega scatter are branch-free.
 struct MechDev {
-  int K, R, nT, Kpad;
-  int r_tb, r_lind, r_troe;
+  int K, R, nT;
+  int r_dup, r_tb, r_lind, r_troe;
   double tedge[MAX_TINT];     // interval t holds tedge[t-1] < T <= tedge[t]; nT-1 finite edges
   const double* W;            // [K]
   const double* invW;         // [K]
   const double* nlo;          // [7][K] NASA-7, T <= t_mid
   const double* nhi;          // [7][K]
   const double* tmid;         // [K]
+  const double* spack;        // [K][16] AoS for smem staging: W, 1/W, t_mid, 0, lo a1..a6, hi a1..a6
   const double* lnA;          // [R]  Eq. 15: ln k_f = lnA + beta lnT - Ta/T
   const double* beta;         // [R]
   const double* Ta;           // [R]  Ea / R_cal
   const double* krc;          // [nT][7][R]  ln k_r = c0 + c1 lnT + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4
-  const int* part;            // [6][R]  slots 0-2 reactants, 3-5 products: (species << 8) | nu ; 0 = empty
+  const int* slot;            // [6][R]  slots 0-2 reactants, 3-5 products (species index or K)
+  const double* rpack;        // [R][rstride] AoS for smem staging: lnA, beta, Ta, slots (6 x 10 bit in the
+                              //   low/high 32-bit words), then per interval 8 doubles: c0..c6, 0
+  int rstride;                // = 4 + 8 nT
   const int* eptr;            // [R - r_tb + 1] CSR of non-unit efficiencies, rows = reactions r_tb..R-1
   const int* espec;
   const double* eval1;        // alpha - 1

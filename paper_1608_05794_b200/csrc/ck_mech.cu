@@ -73,14 +73,29 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   const int nT = (int)edges.size() + 1;
   if (nT > MAX_TINT) { set_error("ck_mech_load: %d distinct t_mid values (max %d)", nT - 1, MAX_TINT - 1); return CK_EUNSUPPORTED; }
 
-  // ---- regroup reactions by type ------------------------------------------------------------------
+  // ---- regroup reactions by type (plain rows: those with six distinct slot species first) ------------
+  auto has_dup = [&](int i) {
+    for (int x = d->reac_ptr[i]; x < d->reac_ptr[i + 1]; ++x) {
+      if (d->reac_nu[x] != 1) return true;
+      for (int y = d->prod_ptr[i]; y < d->prod_ptr[i + 1]; ++y)
+        if (d->prod_spec[y] == d->reac_spec[x]) return true;
+    }
+    for (int y = d->prod_ptr[i]; y < d->prod_ptr[i + 1]; ++y)
+      if (d->prod_nu[y] != 1) return true;
+    return false;
+  };
   std::vector<int> perm;
   int cnt[4] = {0, 0, 0, 0};
-  for (int t = 0; t < 4; ++t)
-    for (int i = 0; i < R; ++i) {
-      if (d->type[i] > 3) { set_error("ck_mech_load: type[%d]=%d", i, (int)d->type[i]); return CK_EINVAL; }
+  int r_dup = 0;
+  for (int i = 0; i < R; ++i) {
+    if (d->type[i] > 3) { set_error("ck_mech_load: type[%d]=%d", i, (int)d->type[i]); return CK_EINVAL; }
+    if (d->reac_ptr[i + 1] < d->reac_ptr[i] || d->prod_ptr[i + 1] < d->prod_ptr[i]) { set_error("ck_mech_load: CSR pointers of reaction %d decrease", i); return CK_EINVAL; }
+  }
+  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
+  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && has_dup(i)) { perm.push_back(i); cnt[0]++; }
+  for (int t = 1; t < 4; ++t)
+    for (int i = 0; i < R; ++i)
       if (d->type[i] == t) { perm.push_back(i); cnt[t]++; }
-    }
   const int r_tb = cnt[0], r_lind = cnt[0] + cnt[1], r_troe = r_lind + cnt[2];
   if (cnt[1] + cnt[2] + cnt[3] > 0 && (!d->eff_ptr)) { set_error("ck_mech_load: eff_ptr missing"); return CK_EINVAL; }
   if (cnt[2] + cnt[3] > 0 && (!d->A0 || !d->beta0 || !d->Ea0)) { set_error("ck_mech_load: low-pressure arrays missing"); return CK_EINVAL; }
@@ -92,7 +107,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     for (int j = 0; j < 7; ++j) { nlo[j * K + k] = d->nasa_lo[7 * k + j]; nhi[j * K + k] = d->nasa_hi[7 * k + j]; }
   }
   std::vector<double> lnA(R), beta(R), Ta(R), krc((size_t)nT * 7 * R);
-  std::vector<int> part(6 * (size_t)std::max(R, 1), 0);
+  std::vector<int> slot(6 * (size_t)std::max(R, 1), K);
   std::vector<int> eptr(1, 0), espec;
   std::vector<double> eval1;
   std::vector<double> lnA0, beta0, Ta0, troe(4 * (size_t)std::max(cnt[3], 1), 0.0);
@@ -112,15 +127,19 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
       const int32_t* nu = side ? d->prod_nu : d->reac_nu;
       const int b = ptr[i], e = ptr[i + 1];
       if (e < b) { set_error("ck_mech_load: CSR pointers of reaction %d decrease", i); return CK_EINVAL; }
-      if (e - b > 3) { set_error("ck_mech_load: reaction %d has %d distinct species on one side (max 3)", i, e - b); return CK_EUNSUPPORTED; }
+      int filled = 0;
       for (int x = b; x < e; ++x) {
-        if (sp[x] < 0 || sp[x] >= K || nu[x] < 1 || nu[x] > 127) { set_error("ck_mech_load: reaction %d: bad species/nu", i); return CK_EINVAL; }
+        if (sp[x] < 0 || sp[x] >= K || nu[x] < 1 || nu[x] > 3) { set_error("ck_mech_load: reaction %d: bad species/nu", i); return (nu[x] > 3) ? CK_EUNSUPPORTED : CK_EINVAL; }
         for (int y = b; y < x; ++y)
           if (sp[y] == sp[x]) { set_error("ck_mech_load: reaction %d lists species %d twice on one side", i, sp[x]); return CK_EINVAL; }
-        part[(size_t)(side * 3 + (x - b)) * R + r] = (sp[x] << 8) | nu[x];
+        for (int c = 0; c < nu[x]; ++c) {
+          if (filled == 3) { set_error("ck_mech_load: reaction %d has molecularity > 3 on one side", i); return CK_EUNSUPPORTED; }
+          slot[(size_t)(side * 3 + filled) * R + r] = sp[x];
+          filled++;
+        }
         net[sp[x]] += side ? nu[x] : -nu[x];
         if (d->elem_comp) for (int el = 0; el < E; ++el) bal[el] += (side ? 1 : -1) * (long long)nu[x] * d->elem_comp[(size_t)sp[x] * E + el];
-        n_part++;
+        n_part += nu[x];
       }
     }
     if (d->elem_comp)
@@ -171,6 +190,24 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
       troe[j] = tp[0]; troe[nt + j] = 1.0 / tp[1]; troe[2 * nt + j] = 1.0 / tp[2]; troe[3 * nt + j] = tp[3];
     }
   }
+  if (K > 1022) { set_error("ck_mech_load: more than 1022 species"); return CK_EUNSUPPORTED; }
+  const int rstride = 4 + 8 * nT;
+  std::vector<double> rpack((size_t)std::max(R, 1) * rstride, 0.0);
+  for (int r = 0; r < R; ++r) {
+    double* q = &rpack[(size_t)r * rstride];
+    q[0] = lnA[r]; q[1] = beta[r]; q[2] = Ta[r];
+    uint32_t w[2] = {0, 0};
+    for (int s = 0; s < 6; ++s) w[s / 3] |= (uint32_t)slot[(size_t)s * R + r] << (10 * (s % 3));
+    std::memcpy(&q[3], w, sizeof w);
+    for (int t = 0; t < nT; ++t)
+      for (int j = 0; j < 7; ++j) q[4 + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];
+  }
+  std::vector<double> spack((size_t)K * 16, 0.0);
+  for (int k = 0; k < K; ++k) {
+    double* q = &spack[(size_t)k * 16];
+    q[0] = W[k]; q[1] = invW[k]; q[2] = tmid[k];
+    for (int j = 0; j < 6; ++j) { q[4 + j] = d->nasa_lo[7 * k + j]; q[10 + j] = d->nasa_hi[7 * k + j]; }
+  }
   std::vector<int> tptr(K + 1, 0), tent;
   for (int k = 0; k < K; ++k) {
     for (auto& pr : tr[k]) tent.push_back((pr.first << 8) | (pr.second + 128));
@@ -180,10 +217,10 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   // ---- arena + upload -------------------------------------------------------------------------------
   Arena a;
   size_t oW = a.put(W), oiW = a.put(invW), olo = a.put(nlo), ohi = a.put(nhi), otm = a.put(tmid);
-  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), opart = a.put(part);
+  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), oslot = a.put(slot), osp = a.put(spack);
   size_t oep = a.put(eptr), oes = a.put(espec), oev = a.put(eval1);
   size_t olnA0 = a.put(lnA0), ob0 = a.put(beta0), oTa0 = a.put(Ta0), otroe = a.put(troe);
-  size_t otp = a.put(tptr), ote = a.put(tent), operm = a.put(perm);
+  size_t otp = a.put(tptr), ote = a.put(tent), operm = a.put(perm), orp = a.put(rpack);
 
   ck_mech* m = new ck_mech;
   m->device = device;
@@ -198,16 +235,17 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   m->arena_bytes = a.buf.size();
   const char* base = (const char*)m->arena;
   MechDev& v = m->dev;
-  v.K = K; v.R = R; v.nT = nT; v.Kpad = K;
-  v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
+  v.K = K; v.R = R; v.nT = nT;
+  v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
   for (int t = 0; t < MAX_TINT; ++t) v.tedge[t] = (t < nT - 1) ? edges[t] : std::numeric_limits<double>::infinity();
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);
   v.nlo = (const double*)(base + olo); v.nhi = (const double*)(base + ohi); v.tmid = (const double*)(base + otm);
   v.lnA = (const double*)(base + olnA); v.beta = (const double*)(base + ob); v.Ta = (const double*)(base + oTa);
-  v.krc = (const double*)(base + okrc); v.part = (const int*)(base + opart);
+  v.krc = (const double*)(base + okrc); v.slot = (const int*)(base + oslot); v.spack = (const double*)(base + osp);
   v.eptr = (const int*)(base + oep); v.espec = (const int*)(base + oes); v.eval1 = (const double*)(base + oev);
   v.lnA0 = (const double*)(base + olnA0); v.beta0 = (const double*)(base + ob0); v.Ta0 = (const double*)(base + oTa0);
   v.troe = (const double*)(base + otroe);
+  v.rpack = (const double*)(base + orp); v.rstride = rstride;
   v.tptr = (const int*)(base + otp); v.tent = (const int*)(base + ote); v.perm = (const int*)(base + operm);
   m->K = K; m->R = R; m->n_tb = cnt[1]; m->n_lind = cnt[2]; m->n_troe = cnt[3]; m->n_rev = n_rev;
   m->n_part = n_part; m->n_eff = (long long)espec.size();
