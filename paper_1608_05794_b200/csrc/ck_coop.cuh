@@ -1,0 +1,220 @@
+// Group-per-reactor (CTA-cooperative) chemistry: one CTA of G threads evaluates the RHS and the analytic
+// Jacobian of ONE reactor whose state lives in shared memory.  Used by ck_jac and the ROS4 step kernel,
+// where the dense N x N matrix must stay on chip.
+//   threads over species  : thermo, concentrations, species sums (gather form, no atomics)
+//   threads over reactions: rates of progress q_i (and their derivatives)
+#pragma once
+#include "ck_chem.cuh"
+
+namespace ck {
+
+// Deterministic CTA-wide sum; `red` is a shared scratch of >= 33 doubles.  All threads get the result.
+template <int G>
+__device__ __forceinline__ double block_sum(double v, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if (G == 32) return v;
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) red[w] = v;
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < G / 32; ++i) s += red[i];
+  return s;
+}
+
+// Shared-memory working set of the cooperative chemistry (pointers into the CTA's dynamic smem)
+struct CoopChem {
+  double* C;     // [K+1] concentrations, C[K] = 1
+  double* cpR;   // [K]
+  double* hRT;   // [K]
+  double* yw;    // [K] Y_k / W_k
+  double* q;     // [R] rates of progress
+  double* w;     // [K] production rates omega_k
+  double* red;   // [40] reduction scratch
+  // Jacobian only:
+  double* dqs;   // [6][R] d q_i / d C_slot (0 for dummy slots)
+  double* dqT;   // [R]    d q_i / d T at constant concentrations
+  double* dqM;   // [R]    d q_i / d [M]_i
+  double* si;    // [R]    sum_m (d q_i/d C_m) C_m
+  double* dns;   // [K]    dense third-body coefficient of row k: sum_i nu_ki dq_i/d[M]_i
+  double* sig;   // [K]    sum_i nu_ki s_i
+  double* tau;   // [K]    sum_i nu_ki dq_i/dT|_C
+};
+struct CoopScalars { double rho, S, cps, Ctot, hw; };
+
+__host__ __device__ inline int coop_chem_doubles(int K, int R, bool jac) {
+  return (K + 1) + 4 * K + R + 40 + (jac ? 9 * R + 3 * K : 0) + 8;
+}
+__device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool jac) {
+  CoopChem c;
+  c.C = base; base += K + 1;
+  c.cpR = base; base += K;
+  c.hRT = base; base += K;
+  c.yw = base; base += K;
+  c.w = base; base += K;
+  c.q = base; base += R;
+  c.red = base; base += 40;
+  c.dqs = base; base += jac ? 6 * R : 0;
+  c.dqT = base; base += jac ? R : 0;
+  c.dqM = base; base += jac ? R : 0;
+  c.si = base; base += jac ? R : 0;
+  c.dns = base; base += jac ? K : 0;
+  c.sig = base; base += jac ? K : 0;
+  c.tau = base;
+  return c;
+}
+
+// f = RHS(y; p) for the reactor whose state is y[0..N) in shared memory; result to fout[0..N) (shared).
+// JAC additionally fills the per-reaction derivative arrays.  Ends with a __syncthreads().
+template <int G, bool JAC>
+__device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* __restrict__ y, double p,
+                                                double* __restrict__ fout, const CoopChem& c, TState& t) {
+  const int K = m.K, R = m.R, tid = threadIdx.x;
+  t = make_tstate(m, y[0]);
+  double Sp = 0.0, cp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    double cpR, hRT;
+    thermo_cp_h(m, k, t, cpR, hRT);
+    const double yw = y[1 + k] * __ldg(m.invW + k);
+    c.cpR[k] = cpR; c.hRT[k] = hRT; c.yw[k] = yw;
+    Sp += yw;
+    cp = fma(yw, cpR, cp);
+  }
+  CoopScalars s;
+  s.S = block_sum<G>(Sp, c.red);
+  s.cps = block_sum<G>(cp, c.red);
+  s.Ctot = p / (R_U * t.T);
+  s.rho = s.Ctot / s.S;
+  for (int k = tid; k < K; k += G) c.C[k] = s.rho * c.yw[k];
+  if (tid == 0) c.C[K] = 1.0;
+  __syncthreads();
+  for (int r = tid; r < R; r += G) {
+    const RxnConst kc = load_rxn_global(m, r, t.tint);
+    RateAux a;
+    const double q = reaction_q<1, JAC>(m, r, kc, t, c.C, s.Ctot, JAC ? &a : nullptr);
+    c.q[r] = q;
+    if (JAC) {
+      const double c0 = c.C[kc.slot[0]], c1 = c.C[kc.slot[1]], c2 = c.C[kc.slot[2]];
+      const double c3 = c.C[kc.slot[3]], c4 = c.C[kc.slot[4]], c5 = c.C[kc.slot[5]];
+      const double gf = a.ci * a.kf, gr = -a.ci * a.kr;
+      double d[6] = {gf * c1 * c2, gf * c0 * c2, gf * c0 * c1, gr * c4 * c5, gr * c3 * c5, gr * c3 * c4};
+      double sum = 0.0;
+#pragma unroll
+      for (int x = 0; x < 6; ++x) {
+        if (kc.slot[x] == K) d[x] = 0.0;
+        c.dqs[(size_t)x * R + r] = d[x];
+        sum = fma(d[x], c.C[kc.slot[x]], sum);
+      }
+      const double net = a.kf * a.pf - a.kr * a.pr;
+      const double dM = a.dci_dM * net;
+      c.dqM[r] = dM;
+      c.dqT[r] = a.ci * (a.kf * a.pf * a.dlnkf_dT - a.kr * a.pr * a.dlnkr_dT) + a.dci_dT * net;
+      // [M]_i = sum_m alpha_im C_m (Ctot = sum C), so sum_m dq/dC_m C_m gains dM * [M]_i
+      double M = 0.0;
+      if (r >= m.r_tb) {
+        const int j = r - m.r_tb;
+        M = s.Ctot;
+        for (int e = __ldg(m.eptr + j), e1 = __ldg(m.eptr + j + 1); e < e1; ++e)
+          M = fma(__ldg(m.eval1 + e), c.C[__ldg(m.espec + e)], M);
+      }
+      c.si[r] = fma(dM, M, sum);
+    }
+  }
+  __syncthreads();
+  const double irho = 1.0 / s.rho;
+  double hwp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    double w = 0.0;
+    for (int e = __ldg(m.tptr + k), e1 = __ldg(m.tptr + k + 1); e < e1; ++e) {
+      const int en = __ldg(m.tent + e);
+      w = fma((double)((en & 255) - 128), c.q[en >> 8], w);
+    }
+    c.w[k] = w;
+    hwp = fma(c.hRT[k], w, hwp);
+    fout[1 + k] = w * __ldg(m.W + k) * irho;
+  }
+  s.hw = block_sum<G>(hwp, c.red);
+  if (tid == 0) fout[0] = -(t.T * s.hw) / (s.rho * s.cps);
+  __syncthreads();
+  return s;
+}
+
+// Analytic Jacobian A[i*lda + j] = d f_i / d y_j (i, j = 0 is T) from the pieces left in shared memory by
+// rhs_coop<G,true>; `f` is that call's output.  Chain rule at constant p:
+//   C_m = rho Y_m / W_m, rho = p/(R_u T S):  dC_m/dT = -C_m/T,  dC_m/dY_j = delta_mj rho/W_j - C_m/(S W_j)
+//   G_kj = sum_i nu_ki dq_i/dC_j,  sigma_k = sum_i nu_ki sum_m dq_i/dC_m C_m,  tau_k = sum_i nu_ki dq_i/dT|_C
+//   d omega_k/dY_j = (rho/W_j) G_kj - sigma_k/(S W_j),   d omega_k/dT = tau_k - sigma_k/T
+// Ends with a __syncthreads().
+template <int G>
+__device__ __forceinline__ void jac_coop(const MechDev& m, const CoopChem& c, const CoopScalars& s, const TState& t,
+                                         const double* __restrict__ f, double* __restrict__ A, int lda) {
+  const int K = m.K, R = m.R, N = K + 1, tid = threadIdx.x;
+  for (int idx = tid; idx < N * lda; idx += G) A[idx] = 0.0;
+  __syncthreads();
+  // rows of G, one thread per species row (no two threads touch the same row)
+  for (int k = tid; k < K; k += G) {
+    double* row = A + (size_t)(1 + k) * lda + 1;
+    double dns = 0.0, sig = 0.0, tau = 0.0;
+    for (int e = __ldg(m.tptr + k), e1 = __ldg(m.tptr + k + 1); e < e1; ++e) {
+      const int en = __ldg(m.tent + e);
+      const int i = en >> 8;
+      const double nu = (double)((en & 255) - 128);
+#pragma unroll
+      for (int x = 0; x < 6; ++x) {
+        const int sl = __ldg(m.slot + (size_t)x * R + i);
+        if (sl != K) row[sl] = fma(nu, c.dqs[(size_t)x * R + i], row[sl]);
+      }
+      sig = fma(nu, c.si[i], sig);
+      tau = fma(nu, c.dqT[i], tau);
+      if (i >= m.r_tb) {
+        const double dM = nu * c.dqM[i];
+        dns += dM;
+        const int j = i - m.r_tb;
+        for (int z = __ldg(m.eptr + j), z1 = __ldg(m.eptr + j + 1); z < z1; ++z) {
+          const int sp = __ldg(m.espec + z);
+          row[sp] = fma(dM, __ldg(m.eval1 + z), row[sp]);
+        }
+      }
+    }
+    c.dns[k] = dns; c.sig[k] = sig; c.tau[k] = tau;
+  }
+  __syncthreads();
+  // scalars of the temperature row
+  double hs = 0.0, ht = 0.0, hcw = 0.0, dcp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    hs = fma(c.hRT[k], c.sig[k], hs);
+    ht = fma(c.hRT[k], c.tau[k] - c.sig[k] * t.invT, ht);
+    hcw = fma((c.cpR[k] - c.hRT[k]) * t.invT, c.w[k], hcw);
+    dcp = fma(c.yw[k], thermo_dcp(m, k, t), dcp);
+  }
+  hs = block_sum<G>(hs, c.red);
+  ht = block_sum<G>(ht, c.red);
+  hcw = block_sum<G>(hcw, c.red);
+  dcp = block_sum<G>(dcp, c.red);
+  const double phi = t.T / (s.rho * s.cps);
+  const double fT = f[0];
+  const double iS = 1.0 / s.S;
+  for (int j = tid; j < K; j += G) {
+    double col = 0.0;
+    for (int k = 0; k < K; ++k) col = fma(c.hRT[k], A[(size_t)(1 + k) * lda + 1 + j] + c.dns[k], col);
+    const double iWj = __ldg(m.invW + j);
+    A[1 + j] = -phi * (s.rho * iWj * col - hs * iS * iWj) + fT * (iS * iWj - c.cpR[j] * iWj / s.cps);
+  }
+  if (tid == 0) A[0] = -phi * (hcw + ht) + fT * (2.0 * t.invT - dcp / s.cps);
+  __syncthreads();
+  // species rows: in-place transform of G into d f_k / d Y_j, and the temperature column
+  const double irho = 1.0 / s.rho;
+  for (int idx = tid; idx < K * K; idx += G) {
+    const int k = idx / K, j = idx - k * K;
+    const double Wk = __ldg(m.W + k), iWj = __ldg(m.invW + j);
+    double* a = A + (size_t)(1 + k) * lda + 1 + j;
+    *a = Wk * iWj * (*a + c.dns[k]) + (f[1 + k] - Wk * irho * c.sig[k]) * iS * iWj;
+  }
+  for (int k = tid; k < K; k += G)
+    A[(size_t)(1 + k) * lda] = __ldg(m.W + k) * irho * (c.tau[k] - c.sig[k] * t.invT) + f[1 + k] * t.invT;
+  __syncthreads();
+}
+
+}  // namespace ck

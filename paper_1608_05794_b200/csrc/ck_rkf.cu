@@ -1,0 +1,282 @@
+// ck_integrate_rkf45: embedded Runge-Kutta-Fehlberg 4(5) (Eq. 2-3; Table B.2
+// with the repaired cells a42 = -7200/2197, a54 = -845/4104, a64 = 1859/4104 -- DESIGN.md reading G3),
+// thread-per-reactor, with the DIVERGENCE-CONTROL LAYER the paper's results call for (PAPER.md:218, 255,
+// 363, 419): a persistent kernel in which every lane is a slot that runs the adaptive driver of
+// Algorithm 1/2 as a small state machine, one RHS evaluation per loop trip, and
+// REFILLS itself from a device-side work queue as soon as its reactor reaches t_f (warp-aggregated
+// atomic fetch), so a reactor that needs 900 attempts never keeps the other 31 lanes of its warp waiting.
+// flags bit 0 switches the refill off (a warp takes 32 consecutive reactors and waits for the slowest, the
+// paper's static mapping) so that both can be measured.  SIMT efficiency = active / issued lane-slots.
+//
+// Per-slot vectors (y_n, k1..k6, stage argument) live in the caller's workspace, component-major over
+// SLOTS (coalesced for every access of the stage loops); the reactor's own column in y_inout is touched
+// twice, at fetch and at completion.
+#include <algorithm>
+#include <vector>
+
+#include "ck_rhs_thread.cuh"
+#include "ck_stats.h"
+
+namespace ck {
+
+// a[s][j]: argument of evaluation s+1 is y + h sum_j a[s][j] k_j ; row 5: 4th-order weights b ; row 6: bhat - b
+__constant__ double RKF_T[7][6] = {
+    {1.0 / 4, 0, 0, 0, 0, 0},
+    {3.0 / 32, 9.0 / 32, 0, 0, 0, 0},
+    {1932.0 / 2197, -7200.0 / 2197, 7296.0 / 2197, 0, 0, 0},
+    {439.0 / 216, -8.0, 3680.0 / 513, -845.0 / 4104, 0, 0},
+    {-8.0 / 27, 2.0, -3544.0 / 2565, 1859.0 / 4104, -11.0 / 40, 0},
+    {25.0 / 216, 0, 1408.0 / 2565, 2197.0 / 4104, -1.0 / 5, 0},
+    {16.0 / 135 - 25.0 / 216, 0, 6656.0 / 12825 - 1408.0 / 2565, 28561.0 / 56430 - 2197.0 / 4104, -9.0 / 50 + 1.0 / 5,
+     2.0 / 55}};
+
+struct RkfArgs {
+  long long n, ld, nslots;
+  double* y;
+  const double* p;
+  double dt, rtol, atol, h0;
+  int max_steps, refill;
+  int *n_accept, *n_reject, *status;
+  double* h_last;
+  int* att;
+  double* V;  // [8][N][nslots]: 0 = y_n, 1..6 = f evaluations, 7 = stage argument
+  DevStats* stats;
+};
+
+enum { ST_H0A = -2, ST_H0B = -1 };  // EstimateH0 evaluations; 0..5 = RK stages
+
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const RkfArgs a) {
+  extern __shared__ double sm[];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int N = m.K + 1;
+  double* Cs = sm + tid;
+  double* wsm = sm + (size_t)(m.K + 1) * BLOCK + tid;
+  double* stage_buf = sm + (size_t)2 * (m.K + 1) * BLOCK;
+  const long long slot = (long long)blockIdx.x * BLOCK + tid;
+  const size_t vs = (size_t)N * a.nslots;  // stride between vectors
+  double* Vy = a.V + slot;                 // component c of vector v: Vy[v*vs + c*nslots]
+  const long long ns = a.nslots;
+
+  long long r = -1;
+  int st = 0, nacc = 0, nrej = 0, status = CK_ST_OK;
+  double t = 0, h = 0, fac_max = 5.0, p = P_0, ha = 0, d1 = 0, h_used = 0;
+  bool last = false;
+  unsigned long long lane_act = 0, lane_tot = 0, c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
+
+  // start an attempt from y_n: step-size guards of Algorithm 1, clip to t_f, stage argument = y_n
+  auto begin_attempt = [&]() -> bool {
+    if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; return false; }
+    if (!isfinite(h)) { status = CK_ST_NONFINITE; return false; }
+    if (h < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; return false; }
+    last = false;
+    if (h >= a.dt - t) { h = a.dt - t; last = true; }
+    for (int c = 0; c < N; ++c) Vy[7 * vs + c * ns] = Vy[c * ns];
+    st = 0;
+    return true;
+  };
+  auto finish = [&]() {
+    for (int c = 0; c < N; ++c) a.y[(size_t)c * a.ld + r] = Vy[c * ns];
+    if (a.n_accept) a.n_accept[r] = nacc;
+    if (a.n_reject) a.n_reject[r] = nrej;
+    if (a.status) a.status[r] = status;
+    if (a.h_last) a.h_last[r] = h_used;
+    a.att[r] = nacc + nrej;
+    c_att += nacc + nrej; c_acc += nacc; c_rej += nrej; c_fail += (status != CK_ST_OK);
+    r = -1;
+  };
+  auto wrms2 = [&](int v, int v2) -> double {  // || V[v] (- V[v2]) || weighted by y_n
+    double s = 0.0;
+    for (int c = 0; c < N; ++c) {
+      double x = Vy[(size_t)v * vs + c * ns];
+      if (v2 >= 0) x -= Vy[(size_t)v2 * vs + c * ns];
+      const double w = x / fma(a.rtol, fabs(Vy[c * ns]), a.atol);
+      s = fma(w, w, s);
+    }
+    return sqrt(s / N);
+  };
+
+  for (;;) {
+    // ---- divergence control: refill idle lanes from the work queue --------------------------------
+    const unsigned idle = __ballot_sync(0xffffffffu, r < 0);
+    if (idle && (a.refill || idle == 0xffffffffu)) {
+      const int cnt = a.refill ? __popc(idle) : 32;
+      unsigned long long base = 0;
+      if (lane == 0) base = atomicAdd(&a.stats->queue, (unsigned long long)cnt);
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (r < 0) {
+        const long long cand = (long long)base + (a.refill ? __popc(idle & ((1u << lane) - 1)) : lane);
+        if (cand < a.n) {
+          r = cand;
+          p = a.p[r];
+          for (int c = 0; c < N; ++c) {
+            const double v = a.y[(size_t)c * a.ld + r];
+            Vy[c * ns] = v;
+            Vy[7 * vs + c * ns] = v;
+          }
+          t = 0; nacc = 0; nrej = 0; status = CK_ST_OK; fac_max = 5.0; h_used = 0; last = false;
+          if (a.h0 > 0.0) { h = a.h0; if (!begin_attempt()) finish(); }
+          else st = ST_H0A;
+        }
+      }
+    }
+    if (!__syncthreads_or(r >= 0)) break;
+    const bool act = r >= 0;
+    lane_act += act; lane_tot += 1;
+    // ---- one RHS evaluation for every lane: f(stage argument) -> evaluation vector of this stage -----
+    const int dstv = (st < 0) ? (st + 3) : (st + 1);  // H0A -> 1, H0B -> 2, stage s -> s+1
+    rhs_thread<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wsm, stage_buf, act);
+    if (!act) continue;
+    c_rhs++;
+    // ---- per-lane state machine ---------------------------------------------------------------------
+    if (st == ST_H0A) {           // EstimateH0, first evaluation: f0 = f(y) (reading G8)
+      const double d0 = wrms2(0, -1);
+      d1 = wrms2(1, -1);
+      ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 * a.dt : 0.01 * d0 / d1;
+      for (int c = 0; c < N; ++c) Vy[7 * vs + c * ns] = fma(ha, Vy[vs + c * ns], Vy[c * ns]);
+      st = ST_H0B;
+    } else if (st == ST_H0B) {    // second evaluation: f(y + ha f0)
+      const double d2 = wrms2(2, 1) / ha;
+      const double dm = fmax(d1, d2);
+      const double hb = (dm <= 1e-15) ? fmax(1e-6 * a.dt, 1e-3 * ha) : pow(0.01 / dm, 0.2);
+      h = fmin(fmin(100.0 * ha, hb), a.dt);
+      if (!begin_attempt()) finish();
+    } else if (st < 5) {          // argument of the next evaluation
+      for (int c = 0; c < N; ++c) {
+        double acc = 0.0;
+#pragma unroll
+        for (int j = 0; j < 5; ++j)
+          if (j <= st) acc = fma(RKF_T[st][j], Vy[(size_t)(j + 1) * vs + c * ns], acc);
+        Vy[7 * vs + c * ns] = fma(h, acc, Vy[c * ns]);
+      }
+      st++;
+    } else {                      // all six evaluations done: 4th-order solution, error, accept / reject
+      double es = 0.0;
+      for (int c = 0; c < N; ++c) {
+        double yb = 0.0, eb = 0.0;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+          const double k = Vy[(size_t)(j + 1) * vs + c * ns];
+          yb = fma(RKF_T[5][j], k, yb);
+          eb = fma(RKF_T[6][j], k, eb);
+        }
+        const double y0 = Vy[c * ns];
+        const double yn = fma(h, yb, y0);
+        Vy[7 * vs + c * ns] = yn;  // candidate kept in the stage-argument vector
+        const double w = (h * eb) / fma(a.rtol, fmax(fabs(y0), fabs(yn)), a.atol);
+        es = fma(w, w, es);
+      }
+      const double err = sqrt(es / N);
+      h_used = h;
+      if (isfinite(err) && err < 1.0) {
+        for (int c = 0; c < N; ++c) Vy[c * ns] = Vy[7 * vs + c * ns];
+        t = last ? a.dt : t + h;
+        nacc++;
+        h *= fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.2)));
+        fac_max = 5.0;
+      } else {
+        nrej++;
+        h *= isfinite(err) ? fmin(1.0, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.2))) : 0.2;
+        fac_max = 1.0;
+      }
+      if (!(t < a.dt) || !begin_attempt()) finish();
+    }
+  }
+  // ---- statistics: one atomic set per warp -------------------------------------------------------------
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    lane_act += __shfl_xor_sync(0xffffffffu, lane_act, o); lane_tot += __shfl_xor_sync(0xffffffffu, lane_tot, o);
+    c_rhs += __shfl_xor_sync(0xffffffffu, c_rhs, o); c_att += __shfl_xor_sync(0xffffffffu, c_att, o);
+    c_acc += __shfl_xor_sync(0xffffffffu, c_acc, o); c_rej += __shfl_xor_sync(0xffffffffu, c_rej, o);
+    c_fail += __shfl_xor_sync(0xffffffffu, c_fail, o);
+  }
+  if (lane == 0) {
+    atomicAdd(&a.stats->lane_active, lane_act); atomicAdd(&a.stats->lane_total, lane_tot);
+    atomicAdd(&a.stats->rhs_evals, c_rhs); atomicAdd(&a.stats->attempts, c_att);
+    atomicAdd(&a.stats->accepted, c_acc); atomicAdd(&a.stats->rejected, c_rej);
+    atomicAdd(&a.stats->failed, c_fail);
+  }
+}
+
+}  // namespace ck
+
+using namespace ck;
+
+namespace ck {
+int32_t integrate_prologue(const char* who, const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double dt,
+                           const ck_opts* o, void* ws, size_t ws_bytes, size_t need, cudaStream_t st);
+int32_t integrate_report(const ck_mech* m, int64_t n, const int32_t* att_dev, const DevStats* stats_dev, int rounds,
+                         long long lu_per_jac, ck_report* rep, cudaStream_t st);
+}
+
+namespace {
+struct RkfPlan { int block = 0; long long grid = 0; size_t smem = 0; };
+
+template <int BLOCK>
+cudaError_t plan_for(const ck_mech* m, long long n, RkfPlan* pl) {
+  pl->block = BLOCK;
+  pl->smem = rhs_smem_bytes(m->K, m->dev.rstride, BLOCK);
+  cudaError_t e = cudaFuncSetAttribute(rkf45_kernel<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
+  if (e != cudaSuccess) return e;
+  int per_sm = 0, sms = 0;
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_kernel<BLOCK>, BLOCK, pl->smem);
+  if (e != cudaSuccess) return e;
+  e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device);
+  if (e != cudaSuccess) return e;
+  pl->grid = std::min<long long>((n + BLOCK - 1) / BLOCK, (long long)std::max(per_sm, 1) * sms);
+  return cudaSuccess;
+}
+
+int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
+  CK_CUDA(cudaSetDevice(m->device));
+  const int block = rhs_pick_block(m->K, m->dev.rstride, n);
+  switch (block) {
+    case 256: CK_CUDA(plan_for<256>(m, n, pl)); break;
+    case 128: CK_CUDA(plan_for<128>(m, n, pl)); break;
+    case 64: CK_CUDA(plan_for<64>(m, n, pl)); break;
+    case 32: CK_CUDA(plan_for<32>(m, n, pl)); break;
+    default: set_error("ck_integrate_rkf45: %d species do not fit the shared-memory columns", m->K); return CK_EUNSUPPORTED;
+  }
+  return CK_OK;
+}
+inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
+}  // namespace
+
+// workspace: [DevStats][int attempts[n]][double V[8][N][nslots]]
+size_t ck_rkf_workspace(const ck_mech* m, int64_t n) {
+  if (n == 0) return sizeof(DevStats);
+  RkfPlan pl;
+  if (rkf_plan(m, n, &pl) != CK_OK) return sizeof(DevStats);  // the integrate call reports the error
+  const size_t nslots = (size_t)pl.grid * pl.block;
+  return sizeof(DevStats) + al256((size_t)n * sizeof(int)) + (size_t)8 * (m->K + 1) * nslots * sizeof(double);
+}
+
+extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt,
+                                      const ck_opts* o, int32_t* n_accept, int32_t* n_reject, int32_t* status,
+                                      double* h_last, void* ws, size_t ws_bytes, ck_report* report, void* stream) {
+  cudaStream_t st = (cudaStream_t)stream;
+  if (!m) { set_error("ck_integrate_rkf45: null mechanism"); return CK_EINVAL; }
+  RkfPlan pl;
+  if (n > 0) { int32_t rc0 = rkf_plan(m, n, &pl); if (rc0) return rc0; }
+  const size_t nslots = (size_t)pl.grid * pl.block;
+  const size_t need = n > 0 ? sizeof(DevStats) + al256((size_t)n * sizeof(int)) + (size_t)8 * (m->K + 1) * nslots * sizeof(double)
+                            : sizeof(DevStats);
+  int32_t rc = integrate_prologue("ck_integrate_rkf45", m, n, y, ld, p, dt, o, ws, ws_bytes, need, st);
+  if (rc) return rc;
+  if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
+  RkfArgs a;
+  a.n = n; a.ld = ld; a.nslots = (long long)nslots; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
+  a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.refill = !(o->flags & 1);
+  a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
+  a.stats = (DevStats*)ws;
+  a.att = (int*)((char*)ws + sizeof(DevStats));
+  a.V = (double*)((char*)ws + sizeof(DevStats) + al256((size_t)n * sizeof(int)));
+  switch (pl.block) {
+    case 256: rkf45_kernel<256><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
+    case 128: rkf45_kernel<128><<<(unsigned)pl.grid, 128, pl.smem, st>>>(m->dev, a); break;
+    case 64: rkf45_kernel<64><<<(unsigned)pl.grid, 64, pl.smem, st>>>(m->dev, a); break;
+    default: rkf45_kernel<32><<<(unsigned)pl.grid, 32, pl.smem, st>>>(m->dev, a); break;
+  }
+  CK_CUDA(cudaGetLastError());
+  return integrate_report(m, n, a.att, a.stats, 1, 0, report, st);
+}
