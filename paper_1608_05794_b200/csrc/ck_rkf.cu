@@ -15,6 +15,7 @@
 #include <vector>
 
 #include "ck_rhs_thread.cuh"
+#include "ck_coop.cuh"
 #include "ck_stats.h"
 
 namespace ck {
@@ -39,6 +40,14 @@ struct RkfArgs {
   int *n_accept, *n_reject, *status;
   double* h_last;
   int* att;
+  // hand-over records of reactors evicted at an attempt boundary (finished by rkf45_coop_kernel)
+  int* elist;           // [n] evicted reactor ids
+  double* rec_t;        // [n] time reached
+  double* rec_h;        // [n] next step size
+  double* rec_fac;      // [n] fac_max (1 right after a reject)
+  int* rec_acc;         // [n]
+  int* rec_rej;         // [n]
+  int evict;            // 1: end-game eviction enabled
   double* V;  // [8][N][nslots]: 0 = y_n, 1..6 = f evaluations, 7 = stage argument
   DevStats* stats;
 };
@@ -61,7 +70,10 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
   long long r = -1;
   int st = 0, nacc = 0, nrej = 0, status = CK_ST_OK;
   double t = 0, h = 0, fac_max = 5.0, p = P_0, ha = 0, d1 = 0, h_used = 0;
-  bool last = false;
+  bool last = false, endgame = false;
+  __shared__ int s_qempty;
+  if (tid == 0) s_qempty = 0;
+  __syncthreads();
   unsigned long long lane_act = 0, lane_tot = 0, c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
 
   // start an attempt from y_n: step-size guards of Algorithm 1, clip to t_f, stage argument = y_n
@@ -69,6 +81,13 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
     if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; return false; }
     if (!isfinite(h)) { status = CK_ST_NONFINITE; return false; }
     if (h < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; return false; }
+    if (endgame) {  // re-batch: hand this reactor to the cooperative finisher (state is at an attempt boundary)
+      for (int c = 0; c < N; ++c) a.y[(size_t)c * a.ld + r] = Vy[c * ns];
+      a.rec_t[r] = t; a.rec_h[r] = h; a.rec_fac[r] = fac_max; a.rec_acc[r] = nacc; a.rec_rej[r] = nrej;
+      a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
+      r = -1;
+      return true;
+    }
     last = false;
     if (h >= a.dt - t) { h = a.dt - t; last = true; }
     for (int c = 0; c < N; ++c) Vy[7 * vs + c * ns] = Vy[c * ns];
@@ -117,10 +136,14 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
           t = 0; nacc = 0; nrej = 0; status = CK_ST_OK; fac_max = 5.0; h_used = 0; last = false;
           if (a.h0 > 0.0) { h = a.h0; if (!begin_attempt()) finish(); }
           else st = ST_H0A;
+        } else {
+          s_qempty = 1;  // the queue ran dry (benign race: every writer stores 1)
         }
       }
     }
-    if (!__syncthreads_or(r >= 0)) break;
+    const int n_active = __syncthreads_count(r >= 0);
+    if (n_active == 0) break;
+    endgame = a.evict && s_qempty && (n_active * 4 < BLOCK);
     const bool act = r >= 0;
     lane_act += act; lane_tot += 1;
     // ---- one RHS evaluation for every lane: f(stage argument) -> evaluation vector of this stage -----
@@ -198,6 +221,96 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
   }
 }
 
+// Finisher of the divergence-control layer: reactors evicted from the thread-per-reactor phase (the
+// stragglers of the step-count distribution) are completed CTA-per-reactor, so that one
+// reactor's long serial chain of attempts runs at the latency of a cooperative RHS (G lanes share one
+// evaluation) instead of holding a mostly idle CTA of the throughput kernel.
+__host__ __device__ inline size_t rkf_coop_smem_doubles(int K, int R) { return (size_t)8 * (K + 1) + coop_chem_doubles(K, R, false); }
+
+template <int G>
+__global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const RkfArgs a) {
+  extern __shared__ double sm[];
+  __shared__ long long s_next;
+  const int N = m.K + 1, tid = threadIdx.x;
+  double* Y = sm;            // y_n
+  double* F = sm + N;        // six evaluation vectors F[j*N + c]
+  double* YT = sm + 7 * N;   // stage argument / candidate
+  const CoopChem c = coop_carve(sm + 8 * N, m.K, m.R, false);
+  const long long n_ev = (long long)a.stats->n_evicted;
+  unsigned long long c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
+  for (;;) {
+    __syncthreads();
+    if (tid == 0) s_next = (long long)atomicAdd(&a.stats->queue2, 1ULL);
+    __syncthreads();
+    if (s_next >= n_ev) break;
+    const long long r = a.elist[s_next];
+    const double p = a.p[r];
+    for (int i = tid; i < N; i += G) Y[i] = a.y[(size_t)i * a.ld + r];
+    double t = a.rec_t[r], h = a.rec_h[r], fac_max = a.rec_fac[r], h_used = 0.0;
+    int nacc = a.rec_acc[r], nrej = a.rec_rej[r], status = CK_ST_OK;
+    __syncthreads();
+    while (t < a.dt) {
+      if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; break; }
+      if (!isfinite(h)) { status = CK_ST_NONFINITE; break; }
+      if (h < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; break; }
+      bool last = false;
+      if (h >= a.dt - t) { h = a.dt - t; last = true; }
+      TState ts;
+      rhs_coop<G, false>(m, Y, p, F, c, ts);
+      for (int s = 0; s < 5; ++s) {
+        for (int i = tid; i < N; i += G) {
+          double acc = 0.0;
+          for (int j = 0; j <= s; ++j) acc = fma(RKF_T[s][j], F[j * N + i], acc);
+          YT[i] = fma(h, acc, Y[i]);
+        }
+        __syncthreads();
+        rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
+      }
+      c_rhs += 6;
+      double es = 0.0;
+      for (int i = tid; i < N; i += G) {
+        double yb = 0.0, eb = 0.0;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) { const double k = F[j * N + i]; yb = fma(RKF_T[5][j], k, yb); eb = fma(RKF_T[6][j], k, eb); }
+        const double yn = fma(h, yb, Y[i]);
+        YT[i] = yn;
+        const double w = (h * eb) / fma(a.rtol, fmax(fabs(Y[i]), fabs(yn)), a.atol);
+        es = fma(w, w, es);
+      }
+      const double err = sqrt(block_sum<G>(es, c.red) / N);
+      h_used = h;
+      if (isfinite(err) && err < 1.0) {
+        __syncthreads();
+        for (int i = tid; i < N; i += G) Y[i] = YT[i];
+        t = last ? a.dt : t + h;
+        nacc++;
+        h *= fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.2)));
+        fac_max = 5.0;
+      } else {
+        nrej++;
+        h *= isfinite(err) ? fmin(1.0, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.2))) : 0.2;
+        fac_max = 1.0;
+      }
+      __syncthreads();
+    }
+    __syncthreads();
+    for (int i = tid; i < N; i += G) a.y[(size_t)i * a.ld + r] = Y[i];
+    if (tid == 0) {
+      if (a.n_accept) a.n_accept[r] = nacc;
+      if (a.n_reject) a.n_reject[r] = nrej;
+      if (a.status) a.status[r] = status;
+      if (a.h_last) a.h_last[r] = h_used;
+      a.att[r] = nacc + nrej;
+    }
+    c_att += nacc + nrej; c_acc += nacc; c_rej += nrej; c_fail += (status != CK_ST_OK);
+  }
+  if (tid == 0) {
+    atomicAdd(&a.stats->rhs_evals, c_rhs); atomicAdd(&a.stats->attempts, c_att);
+    atomicAdd(&a.stats->accepted, c_acc); atomicAdd(&a.stats->rejected, c_rej);
+    atomicAdd(&a.stats->failed, c_fail);
+  }
+}
+
 }  // namespace ck
 
 using namespace ck;
@@ -242,13 +355,14 @@ int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
 inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
 }  // namespace
 
-// workspace: [DevStats][int attempts[n]][double V[8][N][nslots]]
+// workspace: [DevStats][int attempts[n]][hand-over records: 3 int + 3 double per reactor][double V[8][N][nslots]]
 size_t ck_rkf_workspace(const ck_mech* m, int64_t n) {
   if (n == 0) return sizeof(DevStats);
   RkfPlan pl;
   if (rkf_plan(m, n, &pl) != CK_OK) return sizeof(DevStats);  // the integrate call reports the error
   const size_t nslots = (size_t)pl.grid * pl.block;
-  return sizeof(DevStats) + al256((size_t)n * sizeof(int)) + (size_t)8 * (m->K + 1) * nslots * sizeof(double);
+  return sizeof(DevStats) + 4 * al256((size_t)n * sizeof(int)) + 3 * al256((size_t)n * sizeof(double)) +
+         (size_t)8 * (m->K + 1) * nslots * sizeof(double);
 }
 
 extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt,
@@ -259,8 +373,8 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   RkfPlan pl;
   if (n > 0) { int32_t rc0 = rkf_plan(m, n, &pl); if (rc0) return rc0; }
   const size_t nslots = (size_t)pl.grid * pl.block;
-  const size_t need = n > 0 ? sizeof(DevStats) + al256((size_t)n * sizeof(int)) + (size_t)8 * (m->K + 1) * nslots * sizeof(double)
-                            : sizeof(DevStats);
+  const size_t bi = al256((size_t)n * sizeof(int)), bd = al256((size_t)n * sizeof(double));
+  const size_t need = n > 0 ? sizeof(DevStats) + 4 * bi + 3 * bd + (size_t)8 * (m->K + 1) * nslots * sizeof(double) : sizeof(DevStats);
   int32_t rc = integrate_prologue("ck_integrate_rkf45", m, n, y, ld, p, dt, o, ws, ws_bytes, need, st);
   if (rc) return rc;
   if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
@@ -269,8 +383,16 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.refill = !(o->flags & 1);
   a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
   a.stats = (DevStats*)ws;
-  a.att = (int*)((char*)ws + sizeof(DevStats));
-  a.V = (double*)((char*)ws + sizeof(DevStats) + al256((size_t)n * sizeof(int)));
+  char* wp = (char*)ws + sizeof(DevStats);
+  a.att = (int*)wp; wp += bi;
+  a.elist = (int*)wp; wp += bi;
+  a.rec_acc = (int*)wp; wp += bi;
+  a.rec_rej = (int*)wp; wp += bi;
+  a.rec_t = (double*)wp; wp += bd;
+  a.rec_h = (double*)wp; wp += bd;
+  a.rec_fac = (double*)wp; wp += bd;
+  a.V = (double*)wp;
+  a.evict = (o->flags & 3) ? 0 : 1;  // bit 0: static mapping, bit 1: refill only (no finisher)
   switch (pl.block) {
     case 256: rkf45_kernel<256><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
     case 128: rkf45_kernel<128><<<(unsigned)pl.grid, 128, pl.smem, st>>>(m->dev, a); break;
@@ -278,5 +400,28 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
     default: rkf45_kernel<32><<<(unsigned)pl.grid, 32, pl.smem, st>>>(m->dev, a); break;
   }
   CK_CUDA(cudaGetLastError());
-  return integrate_report(m, n, a.att, a.stats, 1, 0, report, st);
+  int rounds = 1;
+  if (a.evict) {  // finisher over the eviction list (its length is read on the device)
+    const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R) * sizeof(double);
+    if (smem2 > 227 * 1024) { set_error("ck_integrate_rkf45: mechanism too large for the cooperative finisher"); return CK_EUNSUPPORTED; }
+    int per_sm = 0, sms = 0;
+    const int N = m->K + 1;
+    CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+    if (N <= 32) {
+      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<32>, 32, smem2));
+      rkf45_coop_kernel<32><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 32, smem2, st>>>(m->dev, a);
+    } else if (N <= 64) {
+      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<64>, 64, smem2));
+      rkf45_coop_kernel<64><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 64, smem2, st>>>(m->dev, a);
+    } else {
+      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<128>, 128, smem2));
+      rkf45_coop_kernel<128><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 128, smem2, st>>>(m->dev, a);
+    }
+    CK_CUDA(cudaGetLastError());
+    rounds = 2;
+  }
+  return integrate_report(m, n, a.att, a.stats, rounds, 0, report, st);
 }

@@ -12,7 +12,10 @@ struct DevStats {
   unsigned long long attempts, accepted, rejected, rhs_evals, jac_evals, failed;
   unsigned long long lane_active;  // lane-slots that did useful work in the step-attempt loop
   unsigned long long lane_total;   // lane-slots issued
-  unsigned long long pad[23];
+  unsigned long long n_evicted;    // reactors handed from the thread-per-reactor phase to the cooperative finisher
+  unsigned long long queue2;       // work-queue head of the finisher
+  unsigned long long qempty;       // set once the main queue ran dry
+  unsigned long long pad[20];
 };
 static_assert(sizeof(DevStats) == 256, "DevStats is the 256-byte header of the workspace");
 
