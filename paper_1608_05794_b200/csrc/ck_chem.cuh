@@ -126,7 +126,8 @@ struct RateAux {
 // Rate of progress q_i of regrouped reaction r.  WANT_AUX also fills the derivative pieces.
 template <int CS, bool WANT_AUX>
 __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnConst& k, const TState& t,
-                                             const double* __restrict__ C, double Ctot, RateAux* aux) {
+                                             const double* __restrict__ C, double Ctot, RateAux* aux,
+                                             const double* __restrict__ xrow = nullptr) {
   const int R = m.R;
   const double beta = k.beta, Ta = k.Ta;
   const double c1 = k.c1, c2 = k.c2, c3 = k.c3, c4 = k.c4, c5 = k.c5, c6 = k.c6;
@@ -137,24 +138,29 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
   if (r >= m.r_tb) {  // third-body / falloff factor c_i (reading G9)
     const int j = r - m.r_tb;
     double M = Ctot;
-    for (int e = __ldg(m.eptr + j), e1 = __ldg(m.eptr + j + 1); e < e1; ++e)
-      M = fma(__ldg(m.eval1 + e), C[(size_t)__ldg(m.espec + e) * CS], M);
+    // constants of this row: from the staged xpack row (shared memory) when given, else from global memory
+    const double* xr = xrow ? xrow : m.xpack + (size_t)j * 16;
+    const unsigned long long xw = (unsigned long long)__double_as_longlong(xr[7]);
+    const int ne = (int)(xw & 15ull);
+    if (ne != 15) {
+      for (int e = 0; e < ne; ++e) M = fma(xr[8 + e], C[(size_t)((xw >> (4 + 10 * e)) & 1023ull) * CS], M);
+    } else {
+      for (int e = __ldg(m.eptr + j), e1 = __ldg(m.eptr + j + 1); e < e1; ++e)
+        M = fma(__ldg(m.eval1 + e), C[(size_t)__ldg(m.espec + e) * CS], M);
+    }
     if (r < m.r_lind) {
       ci = M;
       if (WANT_AUX) dci_dM = 1.0;
     } else {
-      const int jl = r - m.r_lind;
-      const double beta0 = __ldg(m.beta0 + jl), Ta0 = __ldg(m.Ta0 + jl);
-      const double k0 = ck_exp(fma(beta0, t.lnT, __ldg(m.lnA0 + jl)) - Ta0 * t.invT);
+      const double beta0 = xr[1], Ta0 = xr[2];
+      const double k0 = ck_exp(fma(beta0, t.lnT, xr[0]) - Ta0 * t.invT);
       const double k0_kf = k0 / kf;
       const double Pr = k0_kf * M;
       const double inv1p = 1.0 / (1.0 + Pr);
       const double L = Pr * inv1p;  // Lindemann
       double F = 1.0, dlnF_dlP = 0.0, dlnF_dT = 0.0;
       if (r >= m.r_troe) {
-        const int jt = r - m.r_troe, nt = R - m.r_troe;
-        const double a = __ldg(m.troe + jt), i3 = __ldg(m.troe + nt + jt), i1 = __ldg(m.troe + 2 * nt + jt),
-                     T2 = __ldg(m.troe + 3 * nt + jt);
+        const double a = xr[3], i3 = xr[4], i1 = xr[5], T2 = xr[6];
         const double e3 = ck_exp(-T * i3), e1 = ck_exp(-T * i1);
         double Fc = fma(1.0 - a, e3, a * e1);
         double e2 = 0.0;

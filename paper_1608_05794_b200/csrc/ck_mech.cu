@@ -12,15 +12,26 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdarg>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <map>
 
+#include <mutex>
+
 #include "ck_internal.h"
+
+// each translation unit that instantiates rhs_thread has its own constant bank copy (ck_rhs_thread.cuh)
+cudaError_t ck_rhs_cpack_upload(const double* host, size_t n_doubles);
+cudaError_t ck_rkf_cpack_upload(const double* host, size_t n_doubles);
 
 namespace ck {
 
 static thread_local char g_err[512] = "";
+// The constant bank holds the fast reaction rows of ONE mechanism at a time: the first handle loaded while the
+// bank is free owns it until ck_mech_free; other handles run the shared-memory staging path for every row.
+static std::mutex g_const_mu;
+static const ck_mech* g_const_owner = nullptr;
 void set_error(const char* fmt, ...) {
   va_list ap;
   va_start(ap, fmt);
@@ -202,6 +213,19 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     for (int t = 0; t < nT; ++t)
       for (int j = 0; j < 7; ++j) q[4 + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];
   }
+  const int n_special = R - r_tb;
+  std::vector<double> xpack((size_t)std::max(n_special, 1) * 16, 0.0);
+  for (int j = 0; j < n_special; ++j) {
+    double* q = &xpack[(size_t)j * 16];
+    const int r = r_tb + j;
+    if (r >= r_lind) { q[0] = lnA0[r - r_lind]; q[1] = beta0[r - r_lind]; q[2] = Ta0[r - r_lind]; }
+    if (r >= r_troe) { const int jt = r - r_troe, nt = cnt[3]; q[3] = troe[jt]; q[4] = troe[nt + jt]; q[5] = troe[2 * nt + jt]; q[6] = troe[3 * nt + jt]; }
+    const int e0 = eptr[j], ne = eptr[j + 1] - e0;
+    uint64_t w = (ne <= 6) ? (uint64_t)ne : 15u;
+    if (ne <= 6)
+      for (int x = 0; x < ne; ++x) { w |= (uint64_t)espec[e0 + x] << (4 + 10 * x); q[8 + x] = eval1[e0 + x]; }
+    std::memcpy(&q[7], &w, sizeof w);
+  }
   std::vector<double> spack((size_t)K * 16, 0.0);
   for (int k = 0; k < K; ++k) {
     double* q = &spack[(size_t)k * 16];
@@ -217,7 +241,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   // ---- arena + upload -------------------------------------------------------------------------------
   Arena a;
   size_t oW = a.put(W), oiW = a.put(invW), olo = a.put(nlo), ohi = a.put(nhi), otm = a.put(tmid);
-  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), oslot = a.put(slot), osp = a.put(spack);
+  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), oslot = a.put(slot), osp = a.put(spack), oxp = a.put(xpack);
   size_t oep = a.put(eptr), oes = a.put(espec), oev = a.put(eval1);
   size_t olnA0 = a.put(lnA0), ob0 = a.put(beta0), oTa0 = a.put(Ta0), otroe = a.put(troe);
   size_t otp = a.put(tptr), ote = a.put(tent), operm = a.put(perm), orp = a.put(rpack);
@@ -241,12 +265,24 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);
   v.nlo = (const double*)(base + olo); v.nhi = (const double*)(base + ohi); v.tmid = (const double*)(base + otm);
   v.lnA = (const double*)(base + olnA); v.beta = (const double*)(base + ob); v.Ta = (const double*)(base + oTa);
-  v.krc = (const double*)(base + okrc); v.slot = (const int*)(base + oslot); v.spack = (const double*)(base + osp);
+  v.krc = (const double*)(base + okrc); v.slot = (const int*)(base + oslot); v.spack = (const double*)(base + osp); v.xpack = (const double*)(base + oxp);
   v.eptr = (const int*)(base + oep); v.espec = (const int*)(base + oes); v.eval1 = (const double*)(base + oev);
   v.lnA0 = (const double*)(base + olnA0); v.beta0 = (const double*)(base + ob0); v.Ta0 = (const double*)(base + oTa0);
   v.troe = (const double*)(base + otroe);
   v.rpack = (const double*)(base + orp); v.rstride = rstride;
   v.tptr = (const int*)(base + otp); v.tent = (const int*)(base + ote); v.perm = (const int*)(base + operm);
+  v.n_cfast = 0;
+  {
+    const int ncf = std::min(r_dup & ~3, (CPACK_DOUBLES / rstride) & ~3);
+    std::lock_guard<std::mutex> lk(g_const_mu);
+    if (ncf > 0 && g_const_owner == nullptr && getenv("CK_USE_CONST_BANK")) {
+      m->h_rpack.assign(rpack.begin(), rpack.begin() + (size_t)ncf * rstride);
+      cudaError_t e1 = ck_rhs_cpack_upload(m->h_rpack.data(), m->h_rpack.size());
+      if (e1 == cudaSuccess) e1 = ck_rkf_cpack_upload(m->h_rpack.data(), m->h_rpack.size());
+      if (e1 == cudaSuccess) { g_const_owner = m; m->owns_const = true; v.n_cfast = ncf; }
+      else cudaGetLastError();  // fall back to the staging path
+    }
+  }
   m->K = K; m->R = R; m->n_tb = cnt[1]; m->n_lind = cnt[2]; m->n_troe = cnt[3]; m->n_rev = n_rev;
   m->n_part = n_part; m->n_eff = (long long)espec.size();
   *out = m;
@@ -256,6 +292,11 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
 extern "C" int32_t ck_mech_free(ck_mech* m) {
   if (!m) return CK_OK;
   cudaSetDevice(m->device);
+  if (m->owns_const) {
+    cudaDeviceSynchronize();  // no kernel may still be reading this mechanism's rows from the constant bank
+    std::lock_guard<std::mutex> lk(g_const_mu);
+    if (g_const_owner == m) g_const_owner = nullptr;
+  }
   if (m->arena) cudaFree(m->arena);
   if (m->stage) cudaFree(m->stage);
   if (m->hstream) cudaStreamDestroy(m->hstream);

@@ -39,6 +39,8 @@ static int32_t launch_rhs(const ck_mech* m, long long n, const double* y, long l
 
 using namespace ck;
 
+cudaError_t ck_rhs_cpack_upload(const double* host, size_t n_doubles) { return cpack_upload(host, n_doubles); }
+
 extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* dydt,
                           int64_t ld_out, void* stream) {
   if (!m) { set_error("ck_rhs: null mechanism"); return CK_EINVAL; }

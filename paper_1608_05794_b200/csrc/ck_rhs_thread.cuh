@@ -4,9 +4,42 @@
 
 namespace ck {
 
+// Reaction constants of the leading fast rows in the constant bank: read through the uniform datapath, they
+// cost no shared-memory wavefronts (the fast loop was shared-memory-bandwidth bound with staged rows).
+// One copy per translation unit; filled by cpack_upload() when the mechanism owns the bank (ck_mech.cu).
+static __constant__ double c_pack[CPACK_DOUBLES];
+
+static inline cudaError_t cpack_upload(const double* host, size_t n_doubles) {
+  return cudaMemcpyToSymbol(c_pack, host, n_doubles * sizeof(double));
+}
+
+// row `base` (index into c_pack) -> RxnConst; coefficients of both intervals are read uniformly and selected
+// per lane when nT == 2 (the common case), so lanes in different intervals do not serialise the constant cache
+__device__ __forceinline__ RxnConst load_rxn_cpack(int base, int tint, int nT) {
+  RxnConst k;
+  k.lnA = c_pack[base]; k.beta = c_pack[base + 1]; k.Ta = c_pack[base + 2];
+  const double sw = c_pack[base + 3];
+  const unsigned lo = (unsigned)__double2loint(sw), hi = (unsigned)__double2hiint(sw);
+  k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
+  k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  if (nT == 2) {
+    const bool h = tint != 0;
+    k.c0 = h ? c_pack[base + 12] : c_pack[base + 4]; k.c1 = h ? c_pack[base + 13] : c_pack[base + 5];
+    k.c2 = h ? c_pack[base + 14] : c_pack[base + 6]; k.c3 = h ? c_pack[base + 15] : c_pack[base + 7];
+    k.c4 = h ? c_pack[base + 16] : c_pack[base + 8]; k.c5 = h ? c_pack[base + 17] : c_pack[base + 9];
+    k.c6 = h ? c_pack[base + 18] : c_pack[base + 10];
+  } else {
+    const int o = base + 4 + 8 * tint;
+    k.c0 = c_pack[o]; k.c1 = c_pack[o + 1]; k.c2 = c_pack[o + 2]; k.c3 = c_pack[o + 3];
+    k.c4 = c_pack[o + 4]; k.c5 = c_pack[o + 5]; k.c6 = c_pack[o + 6];
+  }
+  return k;
+}
+
 constexpr int RHS_CHUNK = 32;  // reactions (or species) staged per shared-memory chunk
 
-__host__ __device__ inline int rhs_stage_doubles(int rstride) { return RHS_CHUNK * (rstride > 16 ? rstride : 16); }
+// staging buffer: RHS_CHUNK reaction rows (or species rows of 16) + RHS_CHUNK special rows of 16
+__host__ __device__ inline int rhs_stage_doubles(int rstride) { return RHS_CHUNK * ((rstride > 16 ? rstride : 16) + 16); }
 __host__ __device__ inline size_t rhs_smem_bytes(int K, int rstride, int block) {
   return ((size_t)2 * (K + 1) * block + (size_t)rhs_stage_doubles(rstride)) * sizeof(double);
 }
@@ -18,6 +51,36 @@ __device__ __forceinline__ void thermo_row(const double* __restrict__ row, const
   const double a1 = a[0], a2 = a[1], a3 = a[2], a4 = a[3], a5 = a[4], a6 = a[5];
   cpR = fma(fma(fma(fma(a5, T, a4), T, a3), T, a2), T, a1);
   hRT = fma(fma(fma(fma(a5 * 0.2, T, a4 * 0.25), T, a3 * (1.0 / 3.0)), T, a2 * 0.5), T, a1) + a6 * t.invT;
+}
+
+// Four reactions with six distinct slot species each, all in flight: rate constants, products, then the
+// omega scatter with every load issued before the stores.  Slots 1, 2, 4, 5 may hold the dummy index K
+// (warp-uniform): those accesses are predicated off and cost no shared-memory wavefronts.
+template <int BLOCK>
+__device__ __forceinline__ void fast_group(const RxnConst (&kc)[4], const TState& t, int K, const double* __restrict__ Cs,
+                                           double* __restrict__ ws) {
+  double q[4];
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    double kf, kr;
+    rate_constants(kc[u], t, kf, kr);
+    double pf = Cs[kc[u].slot[0] * BLOCK], pr = Cs[kc[u].slot[3] * BLOCK];
+    if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
+    if (kc[u].slot[2] != K) pf *= Cs[kc[u].slot[2] * BLOCK];
+    if (kc[u].slot[4] != K) pr *= Cs[kc[u].slot[4] * BLOCK];
+    if (kc[u].slot[5] != K) pr *= Cs[kc[u].slot[5] * BLOCK];
+    q[u] = fma(kf, pf, -kr * pr);
+  }
+#pragma unroll
+  for (int u = 0; u < 4; ++u) {
+    double w[6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc[u].slot[s] != K) w[s] = ws[kc[u].slot[s] * BLOCK];
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc[u].slot[s] != K) ws[kc[u].slot[s] * BLOCK] = (s < 3) ? w[s] - q[u] : w[s] + q[u];
+  }
 }
 
 // One RHS evaluation for the reactor of this thread; MUST be called by every thread of the CTA (species
@@ -39,7 +102,7 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
     __syncthreads();
     for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
     __syncthreads();
-#pragma unroll 4
+#pragma unroll 8
     for (int j = 0; j < nk; ++j) {
       const double* row = stage + j * 16;
       const double yw = yin[(size_t)(k0 + j + 1) * ldin] * row[1];
@@ -58,40 +121,37 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
   Cs[K * BLOCK] = 1.0;
   ws[K * BLOCK] = 0.0;
   // (3) reactions, chunk by chunk
-  for (int r0 = 0; r0 < R; r0 += RHS_CHUNK) {
+  double* xstage = stage + RHS_CHUNK * (rs > 16 ? rs : 16);
+  // leading fast rows straight from the constant bank (no staging, no barriers)
+  const int ncf = m.n_cfast;
+  for (int r = 0; r < ncf; r += 4) {
+    RxnConst kc[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_cpack((r + u) * rs, t.tint, m.nT);
+    fast_group<BLOCK>(kc, t, K, Cs, ws);
+  }
+  for (int r0 = ncf; r0 < R; r0 += RHS_CHUNK) {
     const int nr = min(RHS_CHUNK, R - r0);
     const double* src = m.rpack + (size_t)r0 * rs;
+    const int x0 = max(r0, m.r_tb);                 // first special row of this chunk
+    const int nx = max(0, r0 + nr - x0);
     __syncthreads();  // previous chunk fully consumed
     for (int idx = tid; idx < nr * rs; idx += BLOCK) stage[idx] = __ldg(src + idx);
+    for (int idx = tid; idx < nx * 16; idx += BLOCK) xstage[idx] = __ldg(m.xpack + (size_t)(x0 - m.r_tb) * 16 + idx);
     __syncthreads();
-    // rows [r0, r0+nfast) have six distinct slot species: two reactions in flight, loads before stores
-    const int nfast = max(0, min(nr, m.r_dup - r0)) & ~1;
-    for (int j = 0; j < nfast; j += 2) {
-      const RxnConst ka = load_rxn_row(stage + j * rs, t.tint);
-      const RxnConst kb = load_rxn_row(stage + (j + 1) * rs, t.tint);
-      double kfa, kra, kfb, krb;
-      rate_constants(ka, t, kfa, kra);
-      rate_constants(kb, t, kfb, krb);
-      const double pfa = Cs[ka.slot[0] * BLOCK] * Cs[ka.slot[1] * BLOCK] * Cs[ka.slot[2] * BLOCK];
-      const double pra = Cs[ka.slot[3] * BLOCK] * Cs[ka.slot[4] * BLOCK] * Cs[ka.slot[5] * BLOCK];
-      const double pfb = Cs[kb.slot[0] * BLOCK] * Cs[kb.slot[1] * BLOCK] * Cs[kb.slot[2] * BLOCK];
-      const double prb = Cs[kb.slot[3] * BLOCK] * Cs[kb.slot[4] * BLOCK] * Cs[kb.slot[5] * BLOCK];
-      const double qa = fma(kfa, pfa, -kra * pra);
-      const double qb = fma(kfb, pfb, -krb * prb);
-      double w[6];
+    // rows [r0, r0+nfast) have six distinct slot species: four reactions in flight, loads before stores
+    const int nfast = max(0, min(nr, m.r_dup - r0)) & ~3;
+    for (int j = 0; j < nfast; j += 4) {
+      RxnConst kc[4];
 #pragma unroll
-      for (int s = 0; s < 6; ++s) w[s] = ws[ka.slot[s] * BLOCK];
-#pragma unroll
-      for (int s = 0; s < 6; ++s) ws[ka.slot[s] * BLOCK] = (s < 3) ? w[s] - qa : w[s] + qa;
-#pragma unroll
-      for (int s = 0; s < 6; ++s) w[s] = ws[kb.slot[s] * BLOCK];
-#pragma unroll
-      for (int s = 0; s < 6; ++s) ws[kb.slot[s] * BLOCK] = (s < 3) ? w[s] - qb : w[s] + qb;
+      for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+      fast_group<BLOCK>(kc, t, K, Cs, ws);
     }
     // remaining rows (repeated species, third-body, falloff): one at a time, sequential scatter
     for (int j = nfast; j < nr; ++j) {
       const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
-      const double q = reaction_q<BLOCK, false>(m, r0 + j, kc, t, Cs, Ctot, nullptr);
+      const int r = r0 + j;
+      const double q = reaction_q<BLOCK, false>(m, r, kc, t, Cs, Ctot, nullptr, xstage + (r >= x0 ? (r - x0) * 16 : 0));
 #pragma unroll
       for (int s = 0; s < 6; ++s) {
         double* w = ws + kc.slot[s] * BLOCK;

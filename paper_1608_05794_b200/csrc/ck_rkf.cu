@@ -315,6 +315,8 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
 
 using namespace ck;
 
+cudaError_t ck_rkf_cpack_upload(const double* host, size_t n_doubles) { return cpack_upload(host, n_doubles); }
+
 namespace ck {
 int32_t integrate_prologue(const char* who, const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double dt,
                            const ck_opts* o, void* ws, size_t ws_bytes, size_t need, cudaStream_t st);
