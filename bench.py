@@ -30,6 +30,7 @@ UNIT = "RHS evals/s"
 # FP64 vector peak derived from unit counts and clocks:
 # 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
 PEAK_SLOTS = 148 * 64 * 1.965e9
+RHS_DRAM_BYTES_PER_STATE = 697.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
 
 
 class ClockSampler:
@@ -89,17 +90,41 @@ def oracle_cores():
 
 
 def time_oracle_rhs(mech, y, p, target_s=12.0):
-    """Oracle RHS on a bounded sample of the workload, all host cores (omp dynamic over states)."""
+    """Oracle RHS (as it stands) on a bounded sample of the workload, all host cores (omp dynamic over states):
+    whole passes over up to 262,144 states are repeated until about `target_s` seconds of CPU work are done."""
     from oracle import ck_oracle
     O = ck_oracle.Mech(mech)
     cores = min(oracle_cores(), ck_oracle.max_threads())
-    ns = 4096
-    t0 = time.perf_counter(); O.rhs(y[:, :ns].copy(), p[:ns].copy(), nthreads=cores); t1 = time.perf_counter()
-    rate = ns / (t1 - t0)
-    ns = int(min(y.shape[1], max(ns, rate * target_s)))
+    ns = int(min(y.shape[1], 262144))
     ys = np.ascontiguousarray(y[:, :ns]); ps = np.ascontiguousarray(p[:ns])
-    t0 = time.perf_counter(); O.rhs(ys, ps, nthreads=cores); t1 = time.perf_counter()
-    return ns / (t1 - t0), cores, ns, t1 - t0
+    O.rhs(ys[:, :4096].copy(), ps[:4096].copy(), nthreads=cores)   # page in / spin up the thread pool
+    done, t0 = 0, time.perf_counter()
+    while True:
+        O.rhs(ys, ps, nthreads=cores)
+        done += ns
+        dt = time.perf_counter() - t0
+        if dt >= target_s:
+            break
+    return done / dt, cores, done, dt
+
+
+def shard_states(y, p, rank):
+    """States of one rank: reactors are independent, so every rank evaluates its own batch (weak scaling);
+    ranks > 0 take a seeded permutation of the same recipe so that no two ranks hold the same column order."""
+    if rank == 0:
+        return y, p
+    perm = np.random.default_rng(1000 + rank).permutation(y.shape[1])
+    return np.ascontiguousarray(y[:, perm]), np.ascontiguousarray(p[perm])
+
+
+def max_over_ranks(value, dist, device=None):
+    """Max of a per-rank timing over the process group (no collective touches the data path)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def run_reference(args):
@@ -118,9 +143,9 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean([d for _, d in vals])), "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": WORKLOAD, "sample": f"{ns} states per step"},
+            "config": {"workload": WORKLOAD, "sample": f"{ns} state evaluations per step"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"{ns} of 1,048,576 states per step, omp dynamic over states"},
+                             "sample": f"{ns} state evaluations per step (passes over 65,536 states of the C2 recipe), omp dynamic over states"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
@@ -178,9 +203,7 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
 
     mech, y, p, cfg = make_config("C2")          # every rank: its own n states (seed offset by rank)
-    if rank:
-        rng = np.random.default_rng(1000 + rank)
-        perm = rng.permutation(y.shape[1]); y = np.ascontiguousarray(y[:, perm]); p = np.ascontiguousarray(p[perm])
+    y, p = shard_states(y, p, rank)
     n = y.shape[1]
     M = ck.Mechanism(mech, device=local)
     yd = torch.from_numpy(y).to(dev); pd = torch.from_numpy(p).to(dev)
@@ -206,8 +229,7 @@ def run_ours(args):
     clk = clocks.stop()
     total_ms = ev[0].elapsed_time(ev[-1])
     per_launch_ms = float(np.mean([ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]))
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, dev)
     value = world * n * args.steps / (total_ms * 1e-3)
 
     # end to end through the host-pointer C-ABI call: pinned host buffers, H2D + kernel + D2H per step
@@ -221,8 +243,7 @@ def run_ours(args):
         M.rhs_host(ynp, pnp, out=onp)
     barrier()
     e2e_s = time.perf_counter() - t0
-    if dist is not None:
-        t = torch.tensor([e2e_s], device=dev); dist.all_reduce(t, op=dist.ReduceOp.MAX); e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
     e2e = {"value": world * n * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(ynp.nbytes + pnp.nbytes),
            "d2h_bytes_per_step": int(onp.nbytes), "steps": e2e_steps}
 
@@ -236,13 +257,9 @@ def run_ours(args):
         measured_peak = ck.fp64_peak(local)
     except Exception:
         pass
-    traffic = None
-    tf = os.path.join(ROOT, "profiles", "rhs_kernel_traffic.json")
-    if os.path.exists(tf):
-        try:
-            traffic = json.load(open(tf)).get("dram_bytes_per_launch")
-        except Exception:
-            pass
+    # dram__bytes_read.sum + dram__bytes_write.sum of ck::rhs_kernel from the ncu --set full capture summarised in
+    # profiles/r01_rhs_kernel_full.md (697 B per state at 262,144 states), scaled to this launch's state count
+    traffic = RHS_DRAM_BYTES_PER_STATE * n
     roofline = {"bound": "alu", "kernel": "ck::rhs_kernel", "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
                 "unit": "TFLOP/s", "frac": achieved / PEAK_SLOTS, "traffic": traffic,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
@@ -260,7 +277,7 @@ def run_ours(args):
             "clocks": clk, "e2e": e2e, "gpu_launches": args.steps,
             "roofline": roofline,
             "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"{ns} of {n} states, one pass, {cpu_dt:.1f} s, omp dynamic over states"}}
+                             "sample": f"{ns} state evaluations (passes over the first 262,144 of {n} states), {cpu_dt:.1f} s, omp dynamic over states"}}
     if args.extras:
         line["integrators"] = integrator_extras(torch, ck, dev)
     print(json.dumps(line))
