@@ -131,6 +131,11 @@ int32_t ck_integrate_host(ck_mech* m, int32_t op, int64_t n, double* y_inout, in
                           const ck_opts* opts, int32_t* n_accept, int32_t* n_reject, int32_t* status, double* h_last,
                           ck_report* report);
 
+/* After ck_integrate_ros: SM cycles spent per phase, summed over CTAs, read back from the workspace `ws` of that
+ * call (device pointer): 0 RHS + reaction derivatives, 1 Jacobian assembly, 2 LU, 3 stage solves, 4 stage RHS,
+ * 5 vectors / control, 6 total.  Synchronises the device. */
+int32_t ck_ros_phase_cycles(const void* ws, int64_t cycles[7]);
+
 /* Roofline support: FP64 instruction count ("slots": DFMA/DMUL/DADD, transcendental at their FP64-pipe
  * instruction counts) that one RHS evaluation of this mechanism needs algorithmically. */
 int32_t ck_rhs_slots(const ck_mech* m, double* slots);

@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version"):
+                     "ck_fp64_peak", "ck_version", "ck_ros_phase_cycles"):
             getattr(L, name).restype = C.c_int32
         _lib = L
     return _lib
@@ -199,6 +199,13 @@ class Mechanism:
                   C.byref(rep) if want_report else None, _stream()))
         return dict(y=y, n_accept=na, n_reject=nr, status=st, h_last=hl, report=rep.as_dict() if want_report else None,
                     ws=ws)
+
+    @staticmethod
+    def ros_phase_cycles(ws):
+        out = (C.c_int64 * 7)()
+        _check(lib().ck_ros_phase_cycles(_ptr(ws), out))
+        names = ("rhs_dq", "jac_assembly", "lu", "solves", "stage_rhs", "vectors_control", "total")
+        return dict(zip(names, [int(v) for v in out]))
 
     # ---- host-pointer entry points (numpy arrays; transfers inside the call) ---------------------------
     def rhs_host(self, y, p, out=None):

@@ -128,3 +128,189 @@ __device__ __forceinline__ void lu_solve_warp(const double* __restrict__ A, int 
 }
 
 }  // namespace ck
+
+// ---------------------------------------------------------------------------------------------------------
+// Register-resident variant for compile-time N <= G (one thread per matrix row, the row in registers):
+// the rank-1 update of step k is N-k register FMAs per thread against the pivot row, which every thread reads
+// as a shared-memory broadcast -- 8 bytes of shared-memory traffic per 32 FMAs instead of 24 bytes per FMA in
+// the shared-memory version above.  Pivoting is IMPLICIT: rows never move; the thread whose row is chosen at
+// step k records pstep = k and drops out of the elimination, so P A = L U holds with P given by pstep.
+// One barrier per step for the broadcast (double-buffered) plus one for the cross-warp argmax.
+namespace ck {
+
+template <int G>
+__device__ __forceinline__ int block_argmax1(double val, int idx, double* red2, int parity) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const double v2 = __shfl_xor_sync(0xffffffffu, val, o);
+    const int i2 = __shfl_xor_sync(0xffffffffu, idx, o);
+    if (v2 > val || (v2 == val && i2 < idx)) { val = v2; idx = i2; }
+  }
+  if (G == 32) return idx;
+  constexpr int W = G / 32;
+  double* rv = red2 + parity * 2 * W;
+  int* ri = reinterpret_cast<int*>(rv + W);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { rv[w] = val; ri[w] = idx; }
+  __syncthreads();
+  double bv = rv[0];
+  int bi = ri[0];
+#pragma unroll
+  for (int i = 1; i < W; ++i) {
+    const double v2 = rv[i];
+    const int i2 = ri[i];
+    if (v2 > bv || (v2 == bv && i2 < bi)) { bv = v2; bi = i2; }
+  }
+  return bi;
+}
+
+// Steps are instantiated by template recursion (compile-time k): nvcc does not fully unroll a 54-trip loop whose
+// body holds another unrolled loop, and a partially unrolled loop would index the row dynamically (local memory).
+template <int N, int G, int K>
+__device__ __forceinline__ void lu_factor_step(double (&a)[N], int& pstep, double* __restrict__ bc, double* red2, bool& ok) {
+  if constexpr (K < N) {
+    const int tid = threadIdx.x;
+    const double v = (pstep == -1) ? fabs(a[K]) : -1.0;
+    const int p = block_argmax1<G>(v, tid, red2, K & 1);
+    double* b = bc + (K & 1) * N;
+    if (tid == p) {
+      pstep = K;
+#pragma unroll
+      for (int j = K; j < N; ++j) b[j] = a[j];
+    }
+    __syncthreads();
+    const double pv = b[K];
+    if (!(fabs(pv) > 0.0) || !isfinite(pv)) ok = false;  // uniform; keep going so that barriers stay aligned
+    const double ipv = 1.0 / pv;
+    if (pstep == -1) {
+      const double l = a[K] * ipv;
+      a[K] = l;
+#pragma unroll
+      for (int j = K + 1; j < N; ++j) a[j] = fma(-l, b[j], a[j]);
+    } else if (pstep == K) {
+      a[K] = ipv;
+    }
+    lu_factor_step<N, G, K + 1>(a, pstep, bc, red2, ok);
+  }
+}
+template <int N, int G, int K>
+__device__ __forceinline__ void lu_fwd_step(const double (&a)[N], int pstep, double& b, double* __restrict__ bs) {
+  if constexpr (K < N) {
+    if (pstep == K) bs[K & 1] = b;
+    __syncthreads();
+    if (pstep > K) b = fma(-a[K], bs[K & 1], b);
+    lu_fwd_step<N, G, K + 1>(a, pstep, b, bs);
+  }
+}
+template <int N, int G, int K>
+__device__ __forceinline__ void lu_bwd_step(const double (&a)[N], int pstep, double& b, double* __restrict__ bs) {
+  if constexpr (K >= 0) {
+    if (pstep == K) { b *= a[K]; bs[K & 1] = b; }
+    __syncthreads();
+    if (pstep >= 0 && pstep < K) b = fma(-a[K], bs[K & 1], b);
+    lu_bwd_step<N, G, K - 1>(a, pstep, b, bs);
+  }
+}
+
+// a: this thread's row (thread tid < N owns row tid).  bc: shared scratch of 2*N doubles; red2: 4*(G/32)+8 doubles.
+// On return a holds L (multipliers, columns < pstep), 1/U_kk at column pstep, U beyond it.  false: zero pivot.
+template <int N, int G>
+__device__ __forceinline__ bool lu_factor_rows(double (&a)[N], int& pstep, double* __restrict__ bc, double* red2) {
+  pstep = (threadIdx.x < N) ? -1 : -2;
+  bool ok = true;
+  lu_factor_step<N, G, 0>(a, pstep, bc, red2, ok);
+  __syncthreads();
+  return ok;
+}
+
+// Solve with the factors left by lu_factor_rows.  b: this thread's right-hand-side entry (row tid) on entry, the
+// solution component x[pstep] on return.  bs: shared scratch of 2 doubles.
+template <int N, int G>
+__device__ __forceinline__ void lu_solve_rows(const double (&a)[N], int pstep, double& b, double* __restrict__ bs) {
+  lu_fwd_step<N, G, 0>(a, pstep, b, bs);       // forward: L y = P b
+  lu_bwd_step<N, G, N - 1>(a, pstep, b, bs);   // backward: U x = y
+  __syncthreads();
+}
+
+}  // namespace ck
+
+// ---------------------------------------------------------------------------------------------------------
+// Generic-N variant of the same scheme with the rows in shared memory (thread tid < N owns row tid, implicit
+// pivoting, runtime N <= G): small code (no unrolling over k), and the rank-1 update is register-blocked eight
+// columns at a time -- all loads issued before the FMAs and stores -- because a one-column-per-trip loop is bound
+// by the shared-memory round trip of each iteration (measured: 100 cycles per FMA).
+// dinv[k] receives 1/U_kk.  The barrier inside block_argmax1 of step k+1 orders step k's row updates before any
+// read of the next pivot row, so there is one barrier per step (G > 32) or a __syncwarp (G == 32).
+namespace ck {
+
+template <int G>
+__device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int lda, int N, int& pstep,
+                                                    double* __restrict__ dinv, double* red2) {
+  const int tid = threadIdx.x;
+  pstep = (tid < N) ? -1 : -2;
+  bool ok = true;
+  double* row = A + (size_t)(tid < N ? tid : 0) * lda;
+  for (int k = 0; k < N; ++k) {
+    const double v = (pstep == -1) ? fabs(row[k]) : -1.0;
+    const int p = block_argmax1<G>(v, tid, red2, k & 1);
+    if (G == 32) __syncwarp();
+    const double* prow = A + (size_t)p * lda;
+    const double pv = prow[k];
+    if (!(fabs(pv) > 0.0) || !isfinite(pv)) ok = false;
+    const double ipv = 1.0 / pv;
+    if (tid == p) { pstep = k; dinv[k] = ipv; }
+    else if (pstep == -1) {
+      const double l = row[k] * ipv;
+      row[k] = l;
+      int j = k + 1;
+      for (; j + 8 <= N; j += 8) {
+        double r[8], u[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) { r[x] = row[j + x]; u[x] = prow[j + x]; }
+#pragma unroll
+        for (int x = 0; x < 8; ++x) row[j + x] = fma(-l, u[x], r[x]);
+      }
+      for (; j < N; ++j) row[j] = fma(-l, prow[j], row[j]);
+    }
+  }
+  __syncthreads();
+  return ok;
+}
+
+// b: entry `tid` of the right-hand side on entry, x[pstep] on return.  bs: 2 doubles of shared scratch.
+template <int G>
+__device__ __forceinline__ void lu_solve_rows_smem(const double* __restrict__ A, int lda, int N, int pstep,
+                                                   const double* __restrict__ dinv, double& b, double* __restrict__ bs) {
+  const double* row = A + (size_t)(threadIdx.x < N ? threadIdx.x : 0) * lda;
+  for (int k0 = 0; k0 < N; k0 += 4) {  // forward: L y = P b ; multipliers prefetched four steps ahead
+    double l[4];
+#pragma unroll
+    for (int x = 0; x < 4; ++x) l[x] = (k0 + x < N) ? row[k0 + x] : 0.0;
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const int k = k0 + x;
+      if (k < N) {
+        if (pstep == k) bs[k & 1] = b;
+        __syncthreads();
+        if (pstep > k) b = fma(-l[x], bs[k & 1], b);
+      }
+    }
+  }
+  for (int k0 = N - 1; k0 >= 0; k0 -= 4) {  // backward: U x = y
+    double u[4];
+#pragma unroll
+    for (int x = 0; x < 4; ++x) u[x] = (k0 - x >= 0) ? row[k0 - x] : 0.0;
+#pragma unroll
+    for (int x = 0; x < 4; ++x) {
+      const int k = k0 - x;
+      if (k >= 0) {
+        if (pstep == k) { b *= dinv[k]; bs[k & 1] = b; }
+        __syncthreads();
+        if (pstep >= 0 && pstep < k) b = fma(-u[x], bs[k & 1], b);
+      }
+    }
+  }
+  __syncthreads();
+}
+
+}  // namespace ck

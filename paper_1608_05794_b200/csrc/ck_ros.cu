@@ -10,6 +10,7 @@
 // controller of DESIGN.md reading G8.  Reactors are handed to CTAs through a device-side work queue (one
 // atomic fetch per reactor), so reactors that need many attempts never hold other reactors' lanes idle.
 #include <algorithm>
+#include <cstdlib>
 #include <vector>
 
 #include "ck_coop.cuh"
@@ -64,14 +65,16 @@ __device__ __forceinline__ double wrms_coop(const double* v, const double* y, in
 // Leaves f(y) in s.f0.  Returns the number of RHS evaluations spent.
 template <int G>
 __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, double p, int mode, double h, double rtol,
-                                             double atol) {
+                                             double atol, long long* clk_mid = nullptr) {
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   TState t;
   if (mode == CK_JAC_ANALYTIC) {
     const CoopScalars sc = rhs_coop<G, true>(m, s.y, p, s.f0, s.c, t);
+    if (clk_mid) *clk_mid = clock64();
     jac_coop<G>(m, s.c, sc, t, s.f0, s.A, lda);
     return 1;
   }
+  if (clk_mid) *clk_mid = clock64();
   rhs_coop<G, false>(m, s.y, p, s.f0, s.c, t);
   const double eps = 2.220446049250313e-16;
   const double fn = wrms_coop<G>(s.f0, s.y, N, rtol, atol, s.c.red);
@@ -145,7 +148,26 @@ __device__ __forceinline__ double estimate_h0_coop(const MechDev& m, RosShared& 
   return fmin(fmin(100.0 * ha, hb), dt);
 }
 
-template <int G, int NR>
+// one stage solve with the register-resident factors: reload this thread's row of L\U from shared memory
+template <int NS, int G>
+__device__ __forceinline__ void solve_rows_smem(const double* __restrict__ A, int lda, int pstep, const double* __restrict__ b_in,
+                                                double* __restrict__ x_out, double* bs) {
+  const int tid = threadIdx.x;
+  double a[NS];
+  if (tid < NS) {
+#pragma unroll
+    for (int j = 0; j < NS; ++j) a[j] = A[(size_t)tid * lda + j];
+  } else {
+#pragma unroll
+    for (int j = 0; j < NS; ++j) a[j] = 0.0;
+  }
+  double b = (tid < NS) ? b_in[tid] : 0.0;
+  lu_solve_rows<NS, G>(a, pstep, b, bs);
+  if (pstep >= 0) x_out[pstep] = b;
+  __syncthreads();
+}
+
+template <int G, int NR, int NS>
 __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs a) {
   using namespace ros4c;
   extern __shared__ double sm[];
@@ -153,6 +175,8 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
   RosShared s = ros_carve(sm, m.K, m.R);
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   long long c_att = 0, c_acc = 0, c_rej = 0, c_rhs = 0, c_jac = 0, c_fail = 0;
+  long long ck[7] = {0, 0, 0, 0, 0, 0, 0};
+  const long long k_begin = clock64();
   long long r = blockIdx.x;
   for (;;) {
     if (a.use_queue) {
@@ -177,37 +201,89 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
       bool last = false;
       if (h >= a.dt - tcur) { h = a.dt - tcur; last = true; }
       // ---- one attempt ----
-      c_rhs += jacobian_coop<G>(m, s, p, a.jac_mode, h, a.rtol, a.atol);
+      long long k0 = clock64(), kmid = k0;
+      c_rhs += jacobian_coop<G>(m, s, p, a.jac_mode, h, a.rtol, a.atol, &kmid);
       c_jac++;
+      long long k1 = clock64();
+      ck[0] += kmid - k0; ck[1] += k1 - kmid;
       const double ihg = 1.0 / (h * gam), ih = 1.0 / h;
       for (int idx = tid; idx < N * lda; idx += G) s.A[idx] = -s.A[idx];
       __syncthreads();
       for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + i] += ihg;
       __syncthreads();
-      const bool ok = lu_factor_block<G>(s.A, lda, N, s.piv, s.c.red);
+      bool ok;
+      int pstep = -2;
+      if constexpr (NS > 0) {  // compile-time N: rows in registers, implicit pivoting (ck_linalg.cuh)
+        double arow[NS];
+        if (tid < NS) {
+#pragma unroll
+          for (int j = 0; j < NS; ++j) arow[j] = s.A[(size_t)tid * lda + j];
+        } else {
+#pragma unroll
+          for (int j = 0; j < NS; ++j) arow[j] = 0.0;
+        }
+        ok = lu_factor_rows<NS, G>(arow, pstep, s.tmp, s.c.red);
+        if (tid < NS) {
+#pragma unroll
+          for (int j = 0; j < NS; ++j) s.A[(size_t)tid * lda + j] = arow[j];
+        }
+        __syncthreads();
+      } else if constexpr (NS < 0) {  // any N <= G: rows in shared memory, implicit pivoting, 8-wide updates
+        ok = lu_factor_rows_smem<G>(s.A, lda, N, pstep, s.e, s.c.red);
+      } else {
+        ok = lu_factor_block<G>(s.A, lda, N, s.piv, s.c.red);
+      }
       if (!ok) { status = CK_ST_ZERO_PIVOT; break; }
+      long long k2 = clock64();
+      ck[2] += k2 - k1;
       TState t;
-      if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.f0, s.u1);
-      __syncthreads();
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 16);
+      else if constexpr (NS < 0) {
+        double bb = (tid < N) ? s.f0[tid] : 0.0;
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        if (pstep >= 0) s.u1[pstep] = bb;
+        __syncthreads();
+      } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.f0, s.u1); __syncthreads(); }
+      long long k3 = clock64();
+      ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = fma(a21, s.u1[i], s.y[i]);
       __syncthreads();
       rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+      k2 = clock64(); ck[4] += k2 - k3;
       for (int i = tid; i < N; i += G) s.rhs[i] = fma(c21 * ih, s.u1[i], s.ft[i]);
       __syncthreads();
-      if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u2);
-      __syncthreads();
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 16);
+      else if constexpr (NS < 0) {
+        double bb = (tid < N) ? s.rhs[tid] : 0.0;
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        if (pstep >= 0) s.u2[pstep] = bb;
+        __syncthreads();
+      } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u2); __syncthreads(); }
+      k3 = clock64(); ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = s.y[i] + a31 * s.u1[i] + a32 * s.u2[i];
       __syncthreads();
       rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+      k2 = clock64(); ck[4] += k2 - k3;
       c_rhs += 2;
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c31 * s.u1[i] + c32 * s.u2[i]) * ih;
       __syncthreads();
-      if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u3);
-      __syncthreads();
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 16);
+      else if constexpr (NS < 0) {
+        double bb = (tid < N) ? s.rhs[tid] : 0.0;
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        if (pstep >= 0) s.u3[pstep] = bb;
+        __syncthreads();
+      } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u3); __syncthreads(); }
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c41 * s.u1[i] + c42 * s.u2[i] + c43 * s.u3[i]) * ih;
       __syncthreads();
-      if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u4);
-      __syncthreads();
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 16);
+      else if constexpr (NS < 0) {
+        double bb = (tid < N) ? s.rhs[tid] : 0.0;
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        if (pstep >= 0) s.u4[pstep] = bb;
+        __syncthreads();
+      } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u4); __syncthreads(); }
+      k3 = clock64(); ck[3] += k3 - k2;
       double es = 0.0;
       for (int i = tid; i < N; i += G) {
         const double yn = s.y[i] + m1 * s.u1[i] + m2 * s.u2[i] + m3 * s.u3[i] + m4 * s.u4[i];
@@ -252,6 +328,9 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
     atomicAdd(&a.stats->rhs_evals, (unsigned long long)c_rhs);
     atomicAdd(&a.stats->jac_evals, (unsigned long long)c_jac);
     atomicAdd(&a.stats->failed, (unsigned long long)c_fail);
+    ck[6] = clock64() - k_begin;
+    ck[5] = ck[6] - (ck[0] + ck[1] + ck[2] + ck[3] + ck[4]);
+    for (int i = 0; i < 7; ++i) atomicAdd(&a.stats->clk[i], (unsigned long long)ck[i]);
   }
 }
 
@@ -277,15 +356,15 @@ int32_t launch_jac(const ck_mech* m, long long n, const double* y, long long ld,
   return CK_OK;
 }
 
-template <int G, int NR>
+template <int G, int NR, int NS>
 int32_t launch_ros(const ck_mech* m, const RosArgs& a, int* grid_out, cudaStream_t st) {
   const size_t smem = ros_smem_doubles(m->K, m->R) * sizeof(double);
-  CK_CUDA(cudaFuncSetAttribute(ros4_kernel<G, NR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CK_CUDA(cudaFuncSetAttribute(ros4_kernel<G, NR, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0, sms = 0;
-  CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros4_kernel<G, NR>, G, smem));
+  CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros4_kernel<G, NR, NS>, G, smem));
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
   const long long grid = std::min<long long>(a.n, (long long)std::max(per_sm, 1) * sms);
-  ros4_kernel<G, NR><<<(unsigned)grid, G, smem, st>>>(m->dev, a);
+  ros4_kernel<G, NR, NS><<<(unsigned)grid, G, smem, st>>>(m->dev, a);
   CK_CUDA(cudaGetLastError());
   *grid_out = (int)grid;
   return CK_OK;
@@ -368,10 +447,16 @@ extern "C" int32_t ck_integrate_ros(const ck_mech* m, int64_t n, double* y, int6
   a.att = att;
   int grid = 0;
   const int NRv = (N + 31) / 32;
-  if (N <= 32) rc = launch_ros<32, 1>(m, a, &grid, st);
-  else if (N <= 64) rc = launch_ros<64, 2>(m, a, &grid, st);
-  else if (NRv <= 4) rc = launch_ros<128, 4>(m, a, &grid, st);
-  else rc = launch_ros<128, 8>(m, a, &grid, st);
+  // compile-time-N instantiations (register-resident LU) for the three model sizes of the paper's Table 1
+  // that fit one row per thread (K = 9 is config 1); any other size runs the generic shared-memory path
+  if (N == 10) rc = launch_ros<32, 1, 10>(m, a, &grid, st);
+  else if (N == 15) rc = launch_ros<32, 1, 15>(m, a, &grid, st);
+  else if (N == 54 && getenv("CK_ROS_REG_LU")) rc = launch_ros<64, 2, 54>(m, a, &grid, st);
+  else if (N <= 32) rc = launch_ros<32, 1, -1>(m, a, &grid, st);
+  else if (N <= 64) rc = launch_ros<64, 2, -1>(m, a, &grid, st);
+  else if (N <= 128) rc = launch_ros<128, 4, -1>(m, a, &grid, st);
+  else if (NRv <= 4) rc = launch_ros<128, 4, 0>(m, a, &grid, st);
+  else rc = launch_ros<128, 8, 0>(m, a, &grid, st);
   if (rc) return rc;
   if (report) {
     rc = integrate_report(m, n, att, a.stats, 1, 1, report, st);
@@ -382,4 +467,13 @@ extern "C" int32_t ck_integrate_ros(const ck_mech* m, int64_t n, double* y, int6
     report->simt_efficiency = 0.5 * (ur + un);
   }
   return rc;
+}
+
+extern "C" int32_t ck_ros_phase_cycles(const void* ws, int64_t cycles[7]) {
+  if (!ws || !cycles) { set_error("ck_ros_phase_cycles: null argument"); return CK_EINVAL; }
+  DevStats hs;
+  CK_CUDA(cudaDeviceSynchronize());
+  CK_CUDA(cudaMemcpy(&hs, ws, sizeof hs, cudaMemcpyDeviceToHost));
+  for (int i = 0; i < 7; ++i) cycles[i] = (int64_t)hs.clk[i];
+  return CK_OK;
 }

@@ -15,7 +15,9 @@ struct DevStats {
   unsigned long long n_evicted;    // reactors handed from the thread-per-reactor phase to the cooperative finisher
   unsigned long long queue2;       // work-queue head of the finisher
   unsigned long long qempty;       // set once the main queue ran dry
-  unsigned long long pad[20];
+  unsigned long long clk[8];       // ROS4 phase clocks (SM cycles summed over CTAs): 0 RHS+dq, 1 Jacobian assembly,
+                                   // 2 LU, 3 solves, 4 stage RHS, 5 vectors/control, 6 total
+  unsigned long long pad[12];
 };
 static_assert(sizeof(DevStats) == 256, "DevStats is the 256-byte header of the workspace");
 
