@@ -41,11 +41,13 @@ struct CoopChem {
   double* dns;   // [K]    dense third-body coefficient of row k: sum_i nu_ki dq_i/d[M]_i
   double* sig;   // [K]    sum_i nu_ki s_i
   double* tau;   // [K]    sum_i nu_ki dq_i/dT|_C
+  int* dsl;      // [6][R] slot species of every reaction (shared-memory copy: the row assembly would otherwise
+                 //        wait on a global load per reaction)
 };
 struct CoopScalars { double rho, S, cps, Ctot, hw; };
 
 __host__ __device__ inline int coop_chem_doubles(int K, int R, bool jac) {
-  return (K + 1) + 4 * K + R + 40 + (jac ? 9 * R + 3 * K : 0) + 8;
+  return (K + 1) + 4 * K + R + 40 + (jac ? 12 * R + 3 * K : 0) + 8;
 }
 __device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool jac) {
   CoopChem c;
@@ -62,7 +64,8 @@ __device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool 
   c.si = base; base += jac ? R : 0;
   c.dns = base; base += jac ? K : 0;
   c.sig = base; base += jac ? K : 0;
-  c.tau = base;
+  c.tau = base; base += jac ? K : 0;
+  c.dsl = reinterpret_cast<int*>(base);
   return c;
 }
 
@@ -105,6 +108,7 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
       for (int x = 0; x < 6; ++x) {
         if (kc.slot[x] == K) d[x] = 0.0;
         c.dqs[(size_t)x * R + r] = d[x];
+        c.dsl[(size_t)x * R + r] = kc.slot[x];
         sum = fma(d[x], c.C[kc.slot[x]], sum);
       }
       const double net = a.kf * a.pf - a.kr * a.pr;
@@ -161,11 +165,23 @@ __device__ __forceinline__ void jac_coop(const MechDev& m, const CoopChem& c, co
       const int en = __ldg(m.tent + e);
       const int i = en >> 8;
       const double nu = (double)((en & 255) - 128);
+      int sl[6];
+      double d[6], rv[6];
 #pragma unroll
-      for (int x = 0; x < 6; ++x) {
-        const int sl = __ldg(m.slot + (size_t)x * R + i);
-        if (sl != K) row[sl] = fma(nu, c.dqs[(size_t)x * R + i], row[sl]);
-      }
+      for (int x = 0; x < 6; ++x) { sl[x] = c.dsl[(size_t)x * R + i]; d[x] = c.dqs[(size_t)x * R + i]; }
+      // a species may sit in two slots (nu = 2, or on both sides): fold the later slot into the earlier one so
+      // that the six row entries can be loaded, updated and stored together (one shared-memory round trip)
+#pragma unroll
+      for (int x = 1; x < 6; ++x)
+#pragma unroll
+        for (int y = 0; y < x; ++y)
+          if (sl[x] == sl[y] && sl[x] != K) { d[y] += d[x]; sl[x] = K; }
+#pragma unroll
+      for (int x = 0; x < 6; ++x)
+        if (sl[x] != K) rv[x] = row[sl[x]];
+#pragma unroll
+      for (int x = 0; x < 6; ++x)
+        if (sl[x] != K) row[sl[x]] = fma(nu, d[x], rv[x]);
       sig = fma(nu, c.si[i], sig);
       tau = fma(nu, c.dqT[i], tau);
       if (i >= m.r_tb) {

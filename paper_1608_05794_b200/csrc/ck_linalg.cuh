@@ -243,6 +243,42 @@ __device__ __forceinline__ void lu_solve_rows(const double (&a)[N], int pstep, d
 // read of the next pivot row, so there is one barrier per step (G > 32) or a __syncwarp (G == 32).
 namespace ck {
 
+// Pivot search with the pivot's reciprocal riding along: `v` = |candidate| (or -1 for rows that are out), `inv` =
+// 1/candidate computed by the caller OFF the critical path.  Warp stage: two REDUX.MAX over the 64-bit pattern of
+// |x| (monotone as an unsigned integer; +1 on the high word so that a live zero still beats a dead row) and a
+// ballot for the first lane holding the maximum; CTA stage: one shared-memory exchange and one barrier.
+// red2: 2 parities x 4 x (G/32) doubles.  Returns the pivot row; *ipv = its reciprocal.
+template <int G>
+__device__ __forceinline__ int block_argmax2(double v, double inv, int idx, double* red2, int parity, double* ipv) {
+  const unsigned hi = (v >= 0.0 || v != v) ? (unsigned)__double2hiint(fabs(v)) + 1u : 0u;
+  const unsigned lo = (unsigned)__double2loint(v);
+  const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+  const unsigned lo2 = (hi == mh) ? lo : 0u;
+  const unsigned ml = __reduce_max_sync(0xffffffffu, lo2);
+  const unsigned win = __ballot_sync(0xffffffffu, hi == mh && lo2 == ml);
+  const int wl = __ffs(win) - 1;
+  int bi = __shfl_sync(0xffffffffu, idx, wl);
+  double binv = __shfl_sync(0xffffffffu, inv, wl);
+  if (G == 32) { *ipv = binv; return bi; }
+  constexpr int W = G / 32;
+  double* base = red2 + parity * 4 * W;
+  unsigned* rk = reinterpret_cast<unsigned*>(base);           // [W][2] keys
+  int* ri = reinterpret_cast<int*>(base + W);                 // [W] rows
+  double* rinv = base + 2 * W;                                // [W] reciprocals
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0) { rk[2 * w] = mh; rk[2 * w + 1] = ml; ri[w] = bi; rinv[w] = binv; }
+  __syncthreads();
+  unsigned bh = rk[0], bl = rk[1];
+  bi = ri[0]; binv = rinv[0];
+#pragma unroll
+  for (int i = 1; i < W; ++i) {
+    const unsigned h2 = rk[2 * i], l2 = rk[2 * i + 1];
+    if (h2 > bh || (h2 == bh && l2 > bl)) { bh = h2; bl = l2; bi = ri[i]; binv = rinv[i]; }
+  }
+  *ipv = binv;
+  return bi;
+}
+
 template <int G>
 __device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int lda, int N, int& pstep,
                                                     double* __restrict__ dinv, double* red2) {
@@ -250,19 +286,25 @@ __device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int 
   pstep = (tid < N) ? -1 : -2;
   bool ok = true;
   double* row = A + (size_t)(tid < N ? tid : 0) * lda;
+  double cand = row[0];
+  double cinv = 1.0 / cand;
   for (int k = 0; k < N; ++k) {
-    const double v = (pstep == -1) ? fabs(row[k]) : -1.0;
-    const int p = block_argmax1<G>(v, tid, red2, k & 1);
+    double ipv;
+    const int p = block_argmax2<G>((pstep == -1) ? fabs(cand) : -1.0, cinv, tid, red2, k & 1, &ipv);
     if (G == 32) __syncwarp();
+    if (!isfinite(ipv) || ipv == 0.0) ok = false;  // zero / non-finite pivot (uniform)
     const double* prow = A + (size_t)p * lda;
-    const double pv = prow[k];
-    if (!(fabs(pv) > 0.0) || !isfinite(pv)) ok = false;
-    const double ipv = 1.0 / pv;
     if (tid == p) { pstep = k; dinv[k] = ipv; }
     else if (pstep == -1) {
-      const double l = row[k] * ipv;
+      const double l = cand * ipv;
       row[k] = l;
       int j = k + 1;
+      if (j < N) {  // next step's candidate and its reciprocal first: they head the next step's critical path
+        cand = fma(-l, prow[j], row[j]);
+        row[j] = cand;
+        cinv = 1.0 / cand;
+        ++j;
+      }
       for (; j + 8 <= N; j += 8) {
         double r[8], u[8];
 #pragma unroll

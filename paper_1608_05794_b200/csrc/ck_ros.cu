@@ -237,10 +237,10 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
       long long k2 = clock64();
       ck[2] += k2 - k1;
       TState t;
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 16);
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 36);
       else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.f0[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
         if (pstep >= 0) s.u1[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.f0, s.u1); __syncthreads(); }
@@ -252,10 +252,10 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
       k2 = clock64(); ck[4] += k2 - k3;
       for (int i = tid; i < N; i += G) s.rhs[i] = fma(c21 * ih, s.u1[i], s.ft[i]);
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 16);
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 36);
       else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
         if (pstep >= 0) s.u2[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u2); __syncthreads(); }
@@ -267,19 +267,19 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
       c_rhs += 2;
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c31 * s.u1[i] + c32 * s.u2[i]) * ih;
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 16);
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 36);
       else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
         if (pstep >= 0) s.u3[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u3); __syncthreads(); }
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c41 * s.u1[i] + c42 * s.u2[i] + c43 * s.u3[i]) * ih;
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 16);
+      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 36);
       else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 16);
+        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
         if (pstep >= 0) s.u4[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u4); __syncthreads(); }
