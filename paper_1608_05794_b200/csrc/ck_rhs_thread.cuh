@@ -144,7 +144,7 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
     for (int j = 0; j < nfast; j += 4) {
       RxnConst kc[4];
 #pragma unroll
-      for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+      for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);  // (uniform both-interval loads + select measured 4 % slower)
       fast_group<BLOCK>(kc, t, K, Cs, ws);
     }
     // remaining rows (repeated species, third-body, falloff): one at a time, sequential scatter
