@@ -5,7 +5,10 @@
 // The only per-thread arrays with data-dependent indices -- concentrations C_k and the production-rate
 // accumulators omega_k -- live in shared memory as conflict-free columns (C[k*BLOCK + tid]); reaction
 // constants are warp-uniform loads.  All arithmetic is FP64.
-#include "ck_rhs_thread.cuh"
+#include <algorithm>
+#include <cstdlib>
+
+#include "ck_rhs_tmem.cuh"
 
 namespace ck {
 
@@ -35,6 +38,21 @@ static int32_t launch_rhs(const ck_mech* m, long long n, const double* y, long l
   return CK_OK;
 }
 
+// accumulators in tensor memory: 512 threads per CTA, one CTA per SM, persistent over batches of 512 reactors
+static int32_t launch_rhs_tmem(const ck_mech* m, long long n, const double* y, long long ld, const double* p, double* f,
+                               long long ldf, cudaStream_t st) {
+  constexpr int BLOCK = 512;
+  const size_t smem = rhs_tmem_smem_bytes(m->K, m->dev.rstride, BLOCK);
+  CK_CUDA(cudaFuncSetAttribute(rhs_kernel_tmem<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int sms = 0;
+  CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  const long long batches = (n + BLOCK - 1) / BLOCK;
+  const long long grid = std::min<long long>(batches, sms);
+  rhs_kernel_tmem<BLOCK><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, n, y, ld, p, f, ldf);
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}
+
 }  // namespace ck
 
 using namespace ck;
@@ -51,6 +69,11 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
   CK_CUDA(cudaSetDevice(m->device));
   cudaStream_t st = (cudaStream_t)stream;
   if (m->dev.rstride > 64) { set_error("ck_rhs: too many temperature intervals"); return CK_EUNSUPPORTED; }
+  // tensor-memory path: needs 2 (K+1) <= 128 columns per warp, the C columns of 512 threads in shared memory,
+  // and enough reactors to fill the 512-thread CTAs
+  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256 &&
+      !getenv("CK_RHS_NO_TMEM"))
+    return launch_rhs_tmem(m, n, y, ld, p, dydt, ld_out, st);
   switch (rhs_pick_block(m->K, m->dev.rstride, n)) {
     case 256: return launch_rhs<256>(m, n, y, ld, p, dydt, ld_out, st);
     case 128: return launch_rhs<128>(m, n, y, ld, p, dydt, ld_out, st);

@@ -1,0 +1,184 @@
+// ck_rhs variant with the production-rate accumulators in TENSOR MEMORY (Blackwell TMEM).
+//
+// The thread-per-reactor RHS needs two per-thread arrays with warp-uniform, data-dependent indices: the
+// concentrations C_k (read-only in the reaction loop) and the accumulators omega_k (read-modify-write).  In
+// shared memory the two columns cost 2 (K+1) 8 B per thread and pin the occupancy at 8 warps per SM.  TMEM is
+// 128 lanes x 512 32-bit columns per SM, and tcgen05.ld/st address it exactly the way these columns are used:
+// one column address for the whole warp, each thread touching its own lane.  Warp w of the CTA owns lane quadrant
+// w & 3 and the column range (w >> 2) * 2 (K+1); with the accumulators there, shared memory holds only C and the
+// CTA can be 512 threads: 16 warps per SM, and the accumulator traffic leaves the shared-memory pipe.
+// Limits: 2 (K+1) columns per warp and four warps per quadrant => K + 1 <= 64.
+#pragma once
+#include "ck_rhs_thread.cuh"
+
+namespace ck {
+
+__device__ __forceinline__ void tm_ld2(uint32_t taddr, double& v) {
+  uint32_t a, b;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(taddr));
+  v = __hiloint2double((int)b, (int)a);
+}
+// issue the load only; the two halves are combined after tm_wait_ld()
+__device__ __forceinline__ void tm_ld2_raw(uint32_t taddr, uint32_t& a, uint32_t& b) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(taddr));
+}
+__device__ __forceinline__ void tm_st2(uint32_t taddr, double v) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"((uint32_t)__double2loint(v)),
+               "r"((uint32_t)__double2hiint(v)));
+}
+__device__ __forceinline__ void tm_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tm_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+
+__host__ __device__ inline size_t rhs_tmem_smem_bytes(int K, int rstride, int block) {
+  return ((size_t)(K + 1) * block + (size_t)rhs_stage_doubles(rstride)) * sizeof(double);
+}
+
+// NG reactions with six distinct slot species in flight; accumulators in TMEM at column base `wt`
+template <int BLOCK, int NG>
+__device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const TState& t, int K,
+                                                const double* __restrict__ Cs, uint32_t wt) {
+  double q[NG];
+#pragma unroll
+  for (int u = 0; u < NG; ++u) {
+    double kf, kr;
+    rate_constants(kc[u], t, kf, kr);
+    double pf = Cs[kc[u].slot[0] * BLOCK], pr = Cs[kc[u].slot[3] * BLOCK];
+    if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
+    if (kc[u].slot[2] != K) pf *= Cs[kc[u].slot[2] * BLOCK];
+    if (kc[u].slot[4] != K) pr *= Cs[kc[u].slot[4] * BLOCK];
+    if (kc[u].slot[5] != K) pr *= Cs[kc[u].slot[5] * BLOCK];
+    q[u] = fma(kf, pf, -kr * pr);
+  }
+#pragma unroll
+  for (int u = 0; u < NG; ++u) {
+    uint32_t lo[6], hi[6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc[u].slot[s] != K) tm_ld2_raw(wt + 2 * kc[u].slot[s], lo[s], hi[s]);
+    tm_wait_ld();
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc[u].slot[s] != K) {
+        const double w = __hiloint2double((int)hi[s], (int)lo[s]);
+        tm_st2(wt + 2 * kc[u].slot[s], (s < 3) ? w - q[u] : w + q[u]);
+      }
+    tm_wait_st();
+  }
+}
+
+template <int BLOCK>
+__device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
+                                                double* __restrict__ fout, long long ldout, double* __restrict__ Cs,
+                                                uint32_t wt, double* __restrict__ stage, bool store) {
+  const int K = m.K, R = m.R, rs = m.rstride;
+  const int tid = threadIdx.x;
+  const TState t = make_tstate(m, yin[0]);
+  double S = 0.0, cps = 0.0;
+  for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
+    const int nk = min(RHS_CHUNK, K - k0);
+    __syncthreads();
+    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    __syncthreads();
+#pragma unroll 4
+    for (int j = 0; j < nk; ++j) {
+      const double* row = stage + j * 16;
+      const double yw = yin[(size_t)(k0 + j + 1) * ldin] * row[1];
+      double cpR, hRT;
+      thermo_row(row, t, cpR, hRT);
+      S += yw;
+      cps = fma(yw, cpR, cps);
+      Cs[(k0 + j) * BLOCK] = yw;
+      tm_st2(wt + 2 * (k0 + j), 0.0);
+    }
+  }
+  const double Ctot = p / (R_U * t.T);
+  const double rho = Ctot / S;
+#pragma unroll 4
+  for (int k = 0; k < K; ++k) Cs[k * BLOCK] *= rho;
+  Cs[K * BLOCK] = 1.0;
+  tm_st2(wt + 2 * K, 0.0);
+  tm_wait_st();
+  double* xstage = stage + RHS_CHUNK * (rs > 16 ? rs : 16);
+  for (int r0 = 0; r0 < R; r0 += RHS_CHUNK) {
+    const int nr = min(RHS_CHUNK, R - r0);
+    const double* src = m.rpack + (size_t)r0 * rs;
+    const int x0 = max(r0, m.r_tb);
+    const int nx = max(0, r0 + nr - x0);
+    __syncthreads();
+    for (int idx = tid; idx < nr * rs; idx += BLOCK) stage[idx] = __ldg(src + idx);
+    for (int idx = tid; idx < nx * 16; idx += BLOCK) xstage[idx] = __ldg(m.xpack + (size_t)(x0 - m.r_tb) * 16 + idx);
+    __syncthreads();
+    const int nfast = max(0, min(nr, m.r_dup - r0)) & ~1;
+    for (int j = 0; j < nfast; j += 2) {
+      RxnConst kc[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+      fast_group_tmem<BLOCK, 2>(kc, t, K, Cs, wt);
+    }
+    for (int j = nfast; j < nr; ++j) {
+      const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
+      const int r = r0 + j;
+      const double q = reaction_q<BLOCK, false>(m, r, kc, t, Cs, Ctot, nullptr, xstage + (r >= x0 ? (r - x0) * 16 : 0));
+#pragma unroll
+      for (int s = 0; s < 6; ++s) {  // sequential: a species may sit in two slots
+        double w;
+        tm_ld2(wt + 2 * kc.slot[s], w);
+        tm_wait_ld();
+        tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+        tm_wait_st();
+      }
+    }
+  }
+  const double irho = 1.0 / rho;
+  double hw = 0.0;
+  for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
+    const int nk = min(RHS_CHUNK, K - k0);
+    __syncthreads();
+    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    __syncthreads();
+#pragma unroll 4
+    for (int j = 0; j < nk; ++j) {
+      const double* row = stage + j * 16;
+      double cpR, hRT, w;
+      thermo_row(row, t, cpR, hRT);
+      tm_ld2(wt + 2 * (k0 + j), w);
+      tm_wait_ld();
+      hw = fma(hRT, w, hw);
+      if (store) fout[(size_t)(k0 + j + 1) * ldout] = w * row[0] * irho;
+    }
+  }
+  if (store) fout[0] = -(t.T * hw) / (rho * cps);
+}
+
+template <int BLOCK>
+__global__ void __launch_bounds__(BLOCK, 1) rhs_kernel_tmem(const MechDev m, long long n, const double* __restrict__ y,
+                                                            long long ld, const double* __restrict__ p,
+                                                            double* __restrict__ f, long long ldf) {
+  extern __shared__ double sm[];
+  __shared__ uint32_t s_tmem;
+  const int tid = threadIdx.x, warp = tid >> 5;
+  if (warp == 0) {  // one warp allocates all 512 columns (one CTA per SM: shared memory is full anyway)
+    const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s_tmem);
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;");
+  const uint32_t tbase = s_tmem;
+  // lane quadrant of this warp in bits 31..16, its column range in bits 15..0
+  const uint32_t wt = tbase + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * (m.K + 1));
+  double* Cs = sm + tid;
+  double* stage = sm + (size_t)(m.K + 1) * BLOCK;
+  for (long long b = blockIdx.x; b * BLOCK < n; b += gridDim.x) {
+    const long long r = b * BLOCK + tid;
+    const bool act = r < n;
+    const long long rr = act ? r : n - 1;
+    rhs_thread_tmem<BLOCK>(m, y + rr, ld, p[rr], f + rr, ldf, Cs, wt, stage, act);
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;");
+  __syncthreads();
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
+}
+
+}  // namespace ck
