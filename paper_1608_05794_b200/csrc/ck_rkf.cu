@@ -14,7 +14,9 @@
 #include <algorithm>
 #include <vector>
 
-#include "ck_rhs_thread.cuh"
+#include <cstdlib>
+
+#include "ck_rhs_tmem.cuh"
 #include "ck_coop.cuh"
 #include "ck_stats.h"
 
@@ -54,14 +56,29 @@ struct RkfArgs {
 
 enum { ST_H0A = -2, ST_H0B = -1 };  // EstimateH0 evaluations; 0..5 = RK stages
 
-template <int BLOCK>
-__global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const RkfArgs a) {
+// TM = true: production-rate accumulators in tensor memory (ck_rhs_tmem.cuh), BLOCK = 512
+template <int BLOCK, bool TM>
+__global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const RkfArgs a) {
   extern __shared__ double sm[];
   const int tid = threadIdx.x, lane = tid & 31;
   const int N = m.K + 1;
   double* Cs = sm + tid;
   double* wsm = sm + (size_t)(m.K + 1) * BLOCK + tid;
-  double* stage_buf = sm + (size_t)2 * (m.K + 1) * BLOCK;
+  double* stage_buf = sm + (size_t)(TM ? 1 : 2) * (m.K + 1) * BLOCK;
+  __shared__ uint32_t s_tmem;
+  uint32_t wt = 0;
+  if (TM) {
+    if (tid < 32) {
+      const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s_tmem);
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst));
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const int warp = tid >> 5;
+    wt = s_tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * (m.K + 1));
+  }
   const long long slot = (long long)blockIdx.x * BLOCK + tid;
   const size_t vs = (size_t)N * a.nslots;  // stride between vectors
   double* Vy = a.V + slot;                 // component c of vector v: Vy[v*vs + c*nslots]
@@ -148,7 +165,8 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
     lane_act += act; lane_tot += 1;
     // ---- one RHS evaluation for every lane: f(stage argument) -> evaluation vector of this stage -----
     const int dstv = (st < 0) ? (st + 3) : (st + 1);  // H0A -> 1, H0B -> 2, stage s -> s+1
-    rhs_thread<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wsm, stage_buf, act);
+    if (TM) rhs_thread_tmem<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wt, stage_buf, act);
+    else rhs_thread<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wsm, stage_buf, act);
     if (!act) continue;
     c_rhs++;
     // ---- per-lane state machine ---------------------------------------------------------------------
@@ -218,6 +236,11 @@ __global__ void __launch_bounds__(BLOCK) rkf45_kernel(const MechDev m, const Rkf
     atomicAdd(&a.stats->rhs_evals, c_rhs); atomicAdd(&a.stats->attempts, c_att);
     atomicAdd(&a.stats->accepted, c_acc); atomicAdd(&a.stats->rejected, c_rej);
     atomicAdd(&a.stats->failed, c_fail);
+  }
+  if (TM) {
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(s_tmem));
   }
 }
 
@@ -325,16 +348,18 @@ int32_t integrate_report(const ck_mech* m, int64_t n, const int32_t* att_dev, co
 }
 
 namespace {
-struct RkfPlan { int block = 0; long long grid = 0; size_t smem = 0; };
+struct RkfPlan { int block = 0; long long grid = 0; size_t smem = 0; bool tmem = false; };
 
-template <int BLOCK>
+template <int BLOCK, bool TM>
 cudaError_t plan_for(const ck_mech* m, long long n, RkfPlan* pl) {
   pl->block = BLOCK;
-  pl->smem = rhs_smem_bytes(m->K, m->dev.rstride, BLOCK);
-  cudaError_t e = cudaFuncSetAttribute(rkf45_kernel<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
+  pl->tmem = TM;
+  pl->smem = TM ? rhs_tmem_smem_bytes(m->K, m->dev.rstride, BLOCK) : rhs_smem_bytes(m->K, m->dev.rstride, BLOCK);
+  cudaError_t e = cudaFuncSetAttribute(rkf45_kernel<BLOCK, TM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl->smem);
   if (e != cudaSuccess) return e;
   int per_sm = 0, sms = 0;
-  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_kernel<BLOCK>, BLOCK, pl->smem);
+  e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_kernel<BLOCK, TM>, BLOCK, pl->smem);
+  if (TM) per_sm = std::min(per_sm, 1);  // one CTA owns all 512 tensor-memory columns
   if (e != cudaSuccess) return e;
   e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device);
   if (e != cudaSuccess) return e;
@@ -344,12 +369,17 @@ cudaError_t plan_for(const ck_mech* m, long long n, RkfPlan* pl) {
 
 int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
   CK_CUDA(cudaSetDevice(m->device));
+  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256 &&
+      !getenv("CK_RHS_NO_TMEM")) {
+    CK_CUDA((plan_for<512, true>(m, n, pl)));
+    return CK_OK;
+  }
   const int block = rhs_pick_block(m->K, m->dev.rstride, n);
   switch (block) {
-    case 256: CK_CUDA(plan_for<256>(m, n, pl)); break;
-    case 128: CK_CUDA(plan_for<128>(m, n, pl)); break;
-    case 64: CK_CUDA(plan_for<64>(m, n, pl)); break;
-    case 32: CK_CUDA(plan_for<32>(m, n, pl)); break;
+    case 256: CK_CUDA((plan_for<256, false>(m, n, pl))); break;
+    case 128: CK_CUDA((plan_for<128, false>(m, n, pl))); break;
+    case 64: CK_CUDA((plan_for<64, false>(m, n, pl))); break;
+    case 32: CK_CUDA((plan_for<32, false>(m, n, pl))); break;
     default: set_error("ck_integrate_rkf45: %d species do not fit the shared-memory columns", m->K); return CK_EUNSUPPORTED;
   }
   return CK_OK;
@@ -396,10 +426,11 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   a.V = (double*)wp;
   a.evict = (o->flags & 3) ? 0 : 1;  // bit 0: static mapping, bit 1: refill only (no finisher)
   switch (pl.block) {
-    case 256: rkf45_kernel<256><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
-    case 128: rkf45_kernel<128><<<(unsigned)pl.grid, 128, pl.smem, st>>>(m->dev, a); break;
-    case 64: rkf45_kernel<64><<<(unsigned)pl.grid, 64, pl.smem, st>>>(m->dev, a); break;
-    default: rkf45_kernel<32><<<(unsigned)pl.grid, 32, pl.smem, st>>>(m->dev, a); break;
+    case 512: rkf45_kernel<512, true><<<(unsigned)pl.grid, 512, pl.smem, st>>>(m->dev, a); break;
+    case 256: rkf45_kernel<256, false><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
+    case 128: rkf45_kernel<128, false><<<(unsigned)pl.grid, 128, pl.smem, st>>>(m->dev, a); break;
+    case 64: rkf45_kernel<64, false><<<(unsigned)pl.grid, 64, pl.smem, st>>>(m->dev, a); break;
+    default: rkf45_kernel<32, false><<<(unsigned)pl.grid, 32, pl.smem, st>>>(m->dev, a); break;
   }
   CK_CUDA(cudaGetLastError());
   int rounds = 1;

@@ -162,3 +162,39 @@ def test_integrate_host_entry_point(oracle):
     assert np.all(r["status"] == 0)
     assert np.all(np.abs(yh[0] - ref["y"][0]) <= 1e-5 * ref["y"][0])
     assert np.all(np.abs(yh[1:] - ref["y"][1:]) <= np.maximum(1e-5 * np.abs(ref["y"][1:]), 1e-10))
+
+
+@pytest.mark.parametrize("name,nsample", [("C3", 256), ("C4", 256), ("C5", 48)])
+def test_full_size_sampled(oracle, name, nsample):
+    """BASELINE configs 3-5 at FULL size, in the launch configuration bench.py times (for C4 that is the
+    tensor-memory variant of the step kernel + the cooperative finisher); reactors are independent, so a seeded
+    sample of columns is integrated one by one by the oracle and compared under the same bounds."""
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+    mech, y, p, cfg = make_config(name)
+    n = y.shape[1]
+    M = ck.Mechanism(mech)
+    yd = torch.from_numpy(y).cuda()
+    res = M.integrate(cfg["call"], yd, torch.from_numpy(p).cuda(), cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"])
+    torch.cuda.synchronize()
+    g = yd.cpu().numpy()
+    assert np.isfinite(g).all() and int(res["report"]["n_failed"]) == 0
+    assert np.all(np.abs(g[1:].sum(0) - 1.0) < 1e-6)               # property at any size
+    idx = np.unique(np.concatenate([np.arange(8), np.arange(n - 8, n),
+                                    np.random.default_rng(11).integers(0, n, nsample)]))
+    O = oracle.Mech(mech)
+    ys = np.ascontiguousarray(y[:, idx]); ps = np.ascontiguousarray(p[idx])
+    ref = O.integrate(cfg["call"], ys, ps, cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"], nthreads=16)
+
+    def tight(rs):
+        if len(rs) == 0:
+            return {}
+        t = O.integrate(cfg["call"], np.ascontiguousarray(ys[:, rs]), np.ascontiguousarray(ps[rs]), cfg["dt"], rtol=1e-9,
+                        atol=1e-13, nthreads=16)
+        return {int(r): t["y"][:, i] for i, r in enumerate(rs)}
+    ti = torch.from_numpy(idx).cuda()
+    st, na, nr = res["status"][ti], res["n_accept"][ti], res["n_reject"][ti]
+    sub = dict(status=st, n_accept=na, n_reject=nr,
+               report=dict(accepted=int(na.sum()), rejected=int(nr.sum()), attempts=int((na + nr).sum()), n_failed=0))
+    _check(g[:, idx], sub, ref, mech["n_species"], tight=tight if cfg["call"] == "rkf45" else None)
