@@ -30,7 +30,7 @@ UNIT = "RHS evals/s"
 # FP64 vector peak derived from unit counts and clocks:
 # 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
 PEAK_SLOTS = 148 * 64 * 1.965e9
-RHS_DRAM_BYTES_PER_STATE = 697.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
+RHS_DRAM_BYTES_PER_STATE = 683.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
 
 
 class ClockSampler:
@@ -258,9 +258,9 @@ def run_ours(args):
     except Exception:
         pass
     # dram__bytes_read.sum + dram__bytes_write.sum of ck::rhs_kernel from the ncu --set full capture summarised in
-    # profiles/r01_rhs_kernel_full.md (697 B per state at 262,144 states), scaled to this launch's state count
+    # profiles/r01_rhs_kernel_full.md (683 B per state at 262,144 states), scaled to this launch's state count
     traffic = RHS_DRAM_BYTES_PER_STATE * n
-    roofline = {"bound": "alu", "kernel": "ck::rhs_kernel", "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
+    roofline = {"bound": "alu", "kernel": "ck::rhs_kernel_tmem<512>", "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
                 "unit": "TFLOP/s", "frac": achieved / PEAK_SLOTS, "traffic": traffic,
                 "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
                 "slots_per_eval": slots, "fp64_pipe_inst_per_s": achieved,
