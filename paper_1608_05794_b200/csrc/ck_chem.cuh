@@ -77,6 +77,7 @@ __device__ __forceinline__ double ck_exp(double x) {
 struct RxnConst {
   double lnA, beta, Ta, c0, c1, c2, c3, c4, c5, c6;
   int slot[6];  // species index (or the dummy K) of the three reactant and three product slots
+  int dup;      // nonzero: a species sits in two slots (scatter slot by slot)
 };
 __device__ __forceinline__ RxnConst load_rxn_global(const MechDev& m, int r, int tint) {
   RxnConst k;
@@ -87,6 +88,7 @@ __device__ __forceinline__ RxnConst load_rxn_global(const MechDev& m, int r, int
   k.c4 = __ldg(c + 4 * (size_t)R); k.c5 = __ldg(c + 5 * (size_t)R); k.c6 = __ldg(c + 6 * (size_t)R);
 #pragma unroll
   for (int s = 0; s < 6; ++s) k.slot[s] = __ldg(m.slot + (size_t)s * R + r);
+  k.dup = 1;
   return k;
 }
 // row = pointer to the reaction's rpack row (shared or global memory, 16-byte aligned).  With two temperature
@@ -101,6 +103,7 @@ __device__ __forceinline__ RxnConst load_rxn_row(const double* row, int tint, in
   const unsigned lo = (unsigned)__double2loint(b.y), hi = (unsigned)__double2hiint(b.y);
   k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
   k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  k.dup = (int)(hi >> 31);
   if (nT == 2) {
     const double2* c = reinterpret_cast<const double2*>(row + 4);
     const double2 l01 = c[0], l23 = c[1], l45 = c[2], l67 = c[3], h01 = c[4], h23 = c[5], h45 = c[6], h67 = c[7];

@@ -209,6 +209,11 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     q[0] = lnA[r]; q[1] = beta[r]; q[2] = Ta[r];
     uint32_t w[2] = {0, 0};
     for (int s = 0; s < 6; ++s) w[s / 3] |= (uint32_t)slot[(size_t)s * R + r] << (10 * (s % 3));
+    bool dup = false;  // a species in two slots: the omega scatter of this row must run slot by slot
+    for (int s = 0; s < 6; ++s)
+      for (int s2 = 0; s2 < s; ++s2)
+        if (slot[(size_t)s * R + r] != K && slot[(size_t)s * R + r] == slot[(size_t)s2 * R + r]) dup = true;
+    if (dup) w[1] |= 0x80000000u;
     std::memcpy(&q[3], w, sizeof w);
     for (int t = 0; t < nT; ++t)
       for (int j = 0; j < 7; ++j) q[4 + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];

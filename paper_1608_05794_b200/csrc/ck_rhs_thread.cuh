@@ -22,6 +22,7 @@ __device__ __forceinline__ RxnConst load_rxn_cpack(int base, int tint, int nT) {
   const unsigned lo = (unsigned)__double2loint(sw), hi = (unsigned)__double2hiint(sw);
   k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
   k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  k.dup = (int)(hi >> 31);
   if (nT == 2) {
     const bool h = tint != 0;
     k.c0 = h ? c_pack[base + 12] : c_pack[base + 4]; k.c1 = h ? c_pack[base + 13] : c_pack[base + 5];
@@ -152,10 +153,20 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
       const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
       const int r = r0 + j;
       const double q = reaction_q<BLOCK, false>(m, r, kc, t, Cs, Ctot, nullptr, xstage + (r >= x0 ? (r - x0) * 16 : 0));
+      if (!kc.dup) {  // six distinct slot species: one round trip
+        double w[6];
 #pragma unroll
-      for (int s = 0; s < 6; ++s) {
-        double* w = ws + kc.slot[s] * BLOCK;
-        *w = (s < 3) ? *w - q : *w + q;
+        for (int s = 0; s < 6; ++s)
+          if (s == 0 || s == 3 || kc.slot[s] != K) w[s] = ws[kc.slot[s] * BLOCK];
+#pragma unroll
+        for (int s = 0; s < 6; ++s)
+          if (s == 0 || s == 3 || kc.slot[s] != K) ws[kc.slot[s] * BLOCK] = (s < 3) ? w[s] - q : w[s] + q;
+      } else {
+#pragma unroll
+        for (int s = 0; s < 6; ++s) {
+          double* w = ws + kc.slot[s] * BLOCK;
+          *w = (s < 3) ? *w - q : *w + q;
+        }
       }
     }
   }

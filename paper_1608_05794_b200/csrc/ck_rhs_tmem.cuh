@@ -119,13 +119,28 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
       const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
       const int r = r0 + j;
       const double q = reaction_q<BLOCK, false>(m, r, kc, t, Cs, Ctot, nullptr, xstage + (r >= x0 ? (r - x0) * 16 : 0));
+      if (!kc.dup) {  // six distinct slot species: one tensor-memory round trip
+        uint32_t lo[6], hi[6];
 #pragma unroll
-      for (int s = 0; s < 6; ++s) {  // sequential: a species may sit in two slots
-        double w;
-        tm_ld2(wt + 2 * kc.slot[s], w);
+        for (int s = 0; s < 6; ++s)
+          if (s == 0 || s == 3 || kc.slot[s] != K) tm_ld2_raw(wt + 2 * kc.slot[s], lo[s], hi[s]);
         tm_wait_ld();
-        tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+#pragma unroll
+        for (int s = 0; s < 6; ++s)
+          if (s == 0 || s == 3 || kc.slot[s] != K) {
+            const double w = __hiloint2double((int)hi[s], (int)lo[s]);
+            tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+          }
         tm_wait_st();
+      } else {
+#pragma unroll
+        for (int s = 0; s < 6; ++s) {  // slot by slot: a species sits in two slots
+          double w;
+          tm_ld2(wt + 2 * kc.slot[s], w);
+          tm_wait_ld();
+          tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+          tm_wait_st();
+        }
       }
     }
   }
