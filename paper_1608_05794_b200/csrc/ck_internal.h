@@ -16,7 +16,7 @@ constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere", PAPER
 constexpr int MAX_TINT = 8;                 // temperature intervals (distinct t_mid values + 1)
 
 // Device view of the packed mechanism (all pointers into one device arena; passed by value to kernels).
-// Reactions are regrouped by type: [0,r_dup) plain with six distinct slot species, [r_dup,r_tb) plain with a
+// Reactions are regrouped by type: [0,r_22) A+B<=>C+D (four distinct species), [r_22,r_dup) other plain rows with distinct slot species, [r_dup,r_tb) plain with a
 // repeated species (nu >= 2 or a species on both sides), [r_tb,r_lind) three-body, [r_lind,r_troe) Lindemann,
 // [r_troe,R) Troe.  Every per-reaction array is SoA over the regrouped index.
 // Stoichiometry is stored as SLOTS: each side of a reaction is expanded to exactly three species indices,
@@ -24,6 +24,7 @@ constexpr int MAX_TINT = 8;                 // temperature intervals (distinct t
 // accumulator at K), so rate products and the omega scatter are branch-free.
 struct MechDev {
   int K, R, nT;
+  int r_22;                   // leading rows of the plain group that are A + B <=> C + D with four distinct species
   int r_dup, r_tb, r_lind, r_troe;
   double tedge[MAX_TINT];     // interval t holds tedge[t-1] < T <= tedge[t]; nT-1 finite edges
   const double* W;            // [K]

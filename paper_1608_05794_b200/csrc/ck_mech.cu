@@ -102,7 +102,10 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     if (d->type[i] > 3) { set_error("ck_mech_load: type[%d]=%d", i, (int)d->type[i]); return CK_EINVAL; }
     if (d->reac_ptr[i + 1] < d->reac_ptr[i] || d->prod_ptr[i + 1] < d->prod_ptr[i]) { set_error("ck_mech_load: CSR pointers of reaction %d decrease", i); return CK_EINVAL; }
   }
-  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
+  auto is22 = [&](int i) { return d->reac_ptr[i + 1] - d->reac_ptr[i] == 2 && d->prod_ptr[i + 1] - d->prod_ptr[i] == 2; };
+  int r_22 = 0;
+  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i) && is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; r_22++; }
+  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i) && !is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
   for (int i = 0; i < R; ++i) if (d->type[i] == 0 && has_dup(i)) { perm.push_back(i); cnt[0]++; }
   for (int t = 1; t < 4; ++t)
     for (int i = 0; i < R; ++i)
@@ -265,7 +268,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   const char* base = (const char*)m->arena;
   MechDev& v = m->dev;
   v.K = K; v.R = R; v.nT = nT;
-  v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
+  v.r_22 = r_22; v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
   for (int t = 0; t < MAX_TINT; ++t) v.tedge[t] = (t < nT - 1) ? edges[t] : std::numeric_limits<double>::infinity();
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);
   v.nlo = (const double*)(base + olo); v.nhi = (const double*)(base + ohi); v.tmid = (const double*)(base + otm);

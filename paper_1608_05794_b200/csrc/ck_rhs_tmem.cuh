@@ -34,7 +34,8 @@ __host__ __device__ inline size_t rhs_tmem_smem_bytes(int K, int rstride, int bl
 }
 
 // NG reactions with six distinct slot species in flight; accumulators in TMEM at column base `wt`
-template <int BLOCK, int NG>
+// B22: every reaction of the group is A + B <=> C + D (slots 0, 1, 3, 4 live, 2 and 5 dummy): no predicates at all
+template <int BLOCK, int NG, bool B22>
 __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const TState& t, int K,
                                                 const double* __restrict__ Cs, uint32_t wt) {
   double q[NG];
@@ -43,10 +44,15 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
     double kf, kr;
     rate_constants(kc[u], t, kf, kr);
     double pf = Cs[kc[u].slot[0] * BLOCK], pr = Cs[kc[u].slot[3] * BLOCK];
-    if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
-    if (kc[u].slot[2] != K) pf *= Cs[kc[u].slot[2] * BLOCK];
-    if (kc[u].slot[4] != K) pr *= Cs[kc[u].slot[4] * BLOCK];
-    if (kc[u].slot[5] != K) pr *= Cs[kc[u].slot[5] * BLOCK];
+    if (B22) {
+      pf *= Cs[kc[u].slot[1] * BLOCK];
+      pr *= Cs[kc[u].slot[4] * BLOCK];
+    } else {
+      if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
+      if (kc[u].slot[2] != K) pf *= Cs[kc[u].slot[2] * BLOCK];
+      if (kc[u].slot[4] != K) pr *= Cs[kc[u].slot[4] * BLOCK];
+      if (kc[u].slot[5] != K) pr *= Cs[kc[u].slot[5] * BLOCK];
+    }
     q[u] = fma(kf, pf, -kr * pr);
   }
 #pragma unroll
@@ -54,11 +60,11 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
     uint32_t lo[6], hi[6];
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (s == 0 || s == 3 || kc[u].slot[s] != K) tm_ld2_raw(wt + 2 * kc[u].slot[s], lo[s], hi[s]);
+      if (B22 ? (s != 2 && s != 5) : (s == 0 || s == 3 || kc[u].slot[s] != K)) tm_ld2_raw(wt + 2 * kc[u].slot[s], lo[s], hi[s]);
     tm_wait_ld();
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (s == 0 || s == 3 || kc[u].slot[s] != K) {
+      if (B22 ? (s != 2 && s != 5) : (s == 0 || s == 3 || kc[u].slot[s] != K)) {
         const double w = __hiloint2double((int)hi[s], (int)lo[s]);
         tm_st2(wt + 2 * kc[u].slot[s], (s < 3) ? w - q[u] : w + q[u]);
       }
@@ -108,12 +114,19 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     for (int idx = tid; idx < nr * rs; idx += BLOCK) stage[idx] = __ldg(src + idx);
     for (int idx = tid; idx < nx * 16; idx += BLOCK) xstage[idx] = __ldg(m.xpack + (size_t)(x0 - m.r_tb) * 16 + idx);
     __syncthreads();
-    const int nfast = max(0, min(nr, m.r_dup - r0)) & ~1;
-    for (int j = 0; j < nfast; j += 2) {
+    const int n22 = max(0, min(nr, m.r_22 - r0)) & ~1;
+    for (int j = 0; j < n22; j += 2) {
       RxnConst kc[2];
 #pragma unroll
       for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
-      fast_group_tmem<BLOCK, 2>(kc, t, K, Cs, wt);
+      fast_group_tmem<BLOCK, 2, true>(kc, t, K, Cs, wt);
+    }
+    const int nfast = n22 + (max(0, min(nr, m.r_dup - r0) - n22) & ~1);
+    for (int j = n22; j < nfast; j += 2) {
+      RxnConst kc[2];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+      fast_group_tmem<BLOCK, 2, false>(kc, t, K, Cs, wt);
     }
     for (int j = nfast; j < nr; ++j) {
       const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
