@@ -114,12 +114,12 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     for (int idx = tid; idx < nr * rs; idx += BLOCK) stage[idx] = __ldg(src + idx);
     for (int idx = tid; idx < nx * 16; idx += BLOCK) xstage[idx] = __ldg(m.xpack + (size_t)(x0 - m.r_tb) * 16 + idx);
     __syncthreads();
-    const int n22 = max(0, min(nr, m.r_22 - r0)) & ~1;
-    for (int j = 0; j < n22; j += 2) {
-      RxnConst kc[2];
+    const int n22 = max(0, min(nr, m.r_22 - r0)) & ~3;
+    for (int j = 0; j < n22; j += 4) {
+      RxnConst kc[4];
 #pragma unroll
-      for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
-      fast_group_tmem<BLOCK, 2, true>(kc, t, K, Cs, wt);
+      for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+      fast_group_tmem<BLOCK, 4, true>(kc, t, K, Cs, wt);
     }
     const int nfast = n22 + (max(0, min(nr, m.r_dup - r0) - n22) & ~1);
     for (int j = n22; j < nfast; j += 2) {
