@@ -13,10 +13,11 @@ namespace ck {
 constexpr double R_U = 8.31446261815324e7;  // erg/(mol K)
 constexpr double R_CAL = 1.98720425864083;  // cal/(mol K)
 constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere")
-constexpr int MAX_TINT = 8;                 // temperature intervals (distinct t_mid values + 1)
+constexpr int MAX_TINT = 8;
+constexpr double T_SAFE_LO = 250.0, T_SAFE_HI = 4500.0;  // window in which the fast rows need no exp range checks                 // temperature intervals (distinct t_mid values + 1)
 
 // Device view of the packed mechanism (all pointers into one device arena; passed by value to kernels).
-// Reactions are regrouped by type: [0,r_22) A+B<=>C+D (four distinct species), [r_22,r_dup) other plain rows with distinct slot species, [r_dup,r_tb) plain with a
+// Reactions are regrouped by type: [0,r_22) A+B<=>C+D (four distinct species), [r_22,r_dup) other plain rows with distinct slot species (both groups: exp arguments bounded, see ck_mech.cu), [r_dup,r_tb) plain with a
 // repeated species (nu >= 2 or a species on both sides), [r_tb,r_lind) three-body, [r_lind,r_troe) Lindemann,
 // [r_troe,R) Troe.  Every per-reaction array is SoA over the regrouped index.
 // Stoichiometry is stored as SLOTS: each side of a reaction is expanded to exactly three species indices,
@@ -26,6 +27,7 @@ struct MechDev {
   int K, R, nT;
   int r_22;                   // leading rows of the plain group that are A + B <=> C + D with four distinct species
   int r_dup, r_tb, r_lind, r_troe;
+  double t_safe_lo, t_safe_hi;  // see ck_mech.cu `bounded`
   double tedge[MAX_TINT];     // interval t holds tedge[t-1] < T <= tedge[t]; nT-1 finite edges
   const double* W;            // [K]
   const double* invW;         // [K]

@@ -102,11 +102,45 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     if (d->type[i] > 3) { set_error("ck_mech_load: type[%d]=%d", i, (int)d->type[i]); return CK_EINVAL; }
     if (d->reac_ptr[i + 1] < d->reac_ptr[i] || d->prod_ptr[i + 1] < d->prod_ptr[i]) { set_error("ck_mech_load: CSR pointers of reaction %d decrease", i); return CK_EINVAL; }
   }
+  // A row may join the fast groups only if the arguments of BOTH of its exponentials stay inside (-680, 680) for
+  // every temperature in [T_SAFE_LO, T_SAFE_HI]: the kernels then evaluate them without range checks whenever
+  // all 32 reactors of a warp are inside that temperature window (ck_exp_nc, ck_chem.cuh).
+  auto bounded = [&](int i) {
+    if (!d->reversible[i] || !(d->A[i] > 0)) return false;
+    std::map<int, int> net;
+    int dnu = 0;
+    for (int x = d->reac_ptr[i]; x < d->reac_ptr[i + 1]; ++x) {
+      if (d->reac_spec[x] < 0 || d->reac_spec[x] >= K) return false;
+      net[d->reac_spec[x]] -= d->reac_nu[x]; dnu -= d->reac_nu[x];
+    }
+    for (int x = d->prod_ptr[i]; x < d->prod_ptr[i + 1]; ++x) {
+      if (d->prod_spec[x] < 0 || d->prod_spec[x] >= K) return false;
+      net[d->prod_spec[x]] += d->prod_nu[x]; dnu += d->prod_nu[x];
+    }
+    const double lnA_ = std::log(d->A[i]), Ta_ = d->Ea[i] / R_CAL;
+    for (int sidx = 0; sidx <= 256; ++sidx) {
+      const double T = T_SAFE_LO * std::pow(T_SAFE_HI / T_SAFE_LO, sidx / 256.0), lnT = std::log(T);
+      const double xf = lnA_ + d->beta[i] * lnT - Ta_ / T;
+      double sum = 0;
+      for (auto& kv : net) {
+        const int k = kv.first;
+        const double* a = (T > d->t_mid[k]) ? &d->nasa_hi[7 * k] : &d->nasa_lo[7 * k];
+        const double g = a[0] * (1 - lnT) - a[1] * T / 2 - a[2] * T * T / 6 - a[3] * T * T * T / 12 - a[4] * T * T * T * T / 20 +
+                         a[5] / T - a[6];
+        sum += kv.second * g;
+      }
+      const double xr = xf - (dnu * std::log(P_0 / (R_U * T)) - sum);
+      if (!(std::fabs(xf) < 680.0) || !(std::fabs(xr) < 680.0)) return false;
+    }
+    return true;
+  };
+  std::vector<char> slow(R, 0);
+  for (int i = 0; i < R; ++i) slow[i] = (d->type[i] != 0) || has_dup(i) || !bounded(i);
   auto is22 = [&](int i) { return d->reac_ptr[i + 1] - d->reac_ptr[i] == 2 && d->prod_ptr[i + 1] - d->prod_ptr[i] == 2; };
   int r_22 = 0;
-  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i) && is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; r_22++; }
-  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && !has_dup(i) && !is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
-  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && has_dup(i)) { perm.push_back(i); cnt[0]++; }
+  for (int i = 0; i < R; ++i) if (!slow[i] && is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; r_22++; }
+  for (int i = 0; i < R; ++i) if (!slow[i] && !is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
+  for (int i = 0; i < R; ++i) if (d->type[i] == 0 && slow[i]) { perm.push_back(i); cnt[0]++; }
   for (int t = 1; t < 4; ++t)
     for (int i = 0; i < R; ++i)
       if (d->type[i] == t) { perm.push_back(i); cnt[t]++; }
@@ -268,6 +302,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   const char* base = (const char*)m->arena;
   MechDev& v = m->dev;
   v.K = K; v.R = R; v.nT = nT;
+  v.t_safe_lo = T_SAFE_LO; v.t_safe_hi = T_SAFE_HI;
   v.r_22 = r_22; v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
   for (int t = 0; t < MAX_TINT; ++t) v.tedge[t] = (t < nT - 1) ? edges[t] : std::numeric_limits<double>::infinity();
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);

@@ -35,14 +35,14 @@ __host__ __device__ inline size_t rhs_tmem_smem_bytes(int K, int rstride, int bl
 
 // NG reactions with six distinct slot species in flight; accumulators in TMEM at column base `wt`
 // B22: every reaction of the group is A + B <=> C + D (slots 0, 1, 3, 4 live, 2 and 5 dummy): no predicates at all
-template <int BLOCK, int NG, bool B22>
+template <int BLOCK, int NG, bool B22, bool NC>
 __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const TState& t, int K,
                                                 const double* __restrict__ Cs, uint32_t wt) {
   double q[NG];
 #pragma unroll
   for (int u = 0; u < NG; ++u) {
     double kf, kr;
-    rate_constants(kc[u], t, kf, kr);
+    rate_constants<NC>(kc[u], t, kf, kr);
     double pf = Cs[kc[u].slot[0] * BLOCK], pr = Cs[kc[u].slot[3] * BLOCK];
     if (B22) {
       pf *= Cs[kc[u].slot[1] * BLOCK];
@@ -72,6 +72,24 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
   }
 }
 
+// fast rows of one staged chunk: [0, n22) four A+B<=>C+D rows at a time, [n22, nfast) two generic rows at a time
+template <int BLOCK, bool NC>
+__device__ __forceinline__ void fast_rows_tmem(const double* __restrict__ stage, int rs, int n22, int nfast, const TState& t,
+                                               int K, const double* __restrict__ Cs, uint32_t wt) {
+  for (int j = 0; j < n22; j += 4) {
+    RxnConst kc[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+    fast_group_tmem<BLOCK, 4, true, NC>(kc, t, K, Cs, wt);
+  }
+  for (int j = n22; j < nfast; j += 2) {
+    RxnConst kc[2];
+#pragma unroll
+    for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+    fast_group_tmem<BLOCK, 2, false, NC>(kc, t, K, Cs, wt);
+  }
+}
+
 template <int BLOCK>
 __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
                                                 double* __restrict__ fout, long long ldout, double* __restrict__ Cs,
@@ -79,6 +97,8 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
   const int K = m.K, R = m.R, rs = m.rstride;
   const int tid = threadIdx.x;
   const TState t = make_tstate(m, yin[0]);
+  // every reactor of the warp inside the window for which the packer bounded the fast rows' exp arguments?
+  const bool allsafe = __all_sync(0xffffffffu, t.T >= m.t_safe_lo && t.T <= m.t_safe_hi);
   double S = 0.0, cps = 0.0;
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
@@ -115,19 +135,9 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     for (int idx = tid; idx < nx * 16; idx += BLOCK) xstage[idx] = __ldg(m.xpack + (size_t)(x0 - m.r_tb) * 16 + idx);
     __syncthreads();
     const int n22 = max(0, min(nr, m.r_22 - r0)) & ~3;
-    for (int j = 0; j < n22; j += 4) {
-      RxnConst kc[4];
-#pragma unroll
-      for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
-      fast_group_tmem<BLOCK, 4, true>(kc, t, K, Cs, wt);
-    }
     const int nfast = n22 + (max(0, min(nr, m.r_dup - r0) - n22) & ~1);
-    for (int j = n22; j < nfast; j += 2) {
-      RxnConst kc[2];
-#pragma unroll
-      for (int u = 0; u < 2; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
-      fast_group_tmem<BLOCK, 2, false>(kc, t, K, Cs, wt);
-    }
+    if (allsafe) fast_rows_tmem<BLOCK, true>(stage, rs, n22, nfast, t, K, Cs, wt);
+    else fast_rows_tmem<BLOCK, false>(stage, rs, n22, nfast, t, K, Cs, wt);
     for (int j = nfast; j < nr; ++j) {
       const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
       const int r = r0 + j;

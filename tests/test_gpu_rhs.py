@@ -84,3 +84,22 @@ def test_rhs_host_entry_point(oracle):
     f = M.rhs_host(y, p)
     fd = M.rhs(torch.from_numpy(y).cuda(), torch.from_numpy(p).cuda()).cpu().numpy()
     assert np.array_equal(f, fd)
+
+
+def test_rhs_temperature_outside_safe_window(oracle):
+    """Warps holding a reactor outside the temperature window for which the packer bounded the exponentials'
+    arguments (250..4500 K) take the range-checked path; exercised at a size that runs the tensor-memory kernel."""
+    from synth_inputs import make_config
+    mech, y, p, _ = make_config("C2", n=40000)
+    y = y.copy()
+    y[0, 5::64] = 205.0
+    y[0, 37::64] = 4950.0
+    M, torch = _gpu(mech)
+    f = M.rhs(torch.from_numpy(y).cuda(), torch.from_numpy(p).cuda()).cpu().numpy()
+    idx = np.unique(np.concatenate([np.arange(0, 192), np.arange(5, 40000, 640), np.arange(37, 40000, 640)]))
+    O = oracle.Mech(mech)
+    ys = np.ascontiguousarray(y[:, idx]); ps = np.ascontiguousarray(p[idx])
+    fref = O.rhs(ys, ps, prec=1, nthreads=8)
+    _, D = O.rhs(ys, ps, want_scale=True, nthreads=8)
+    assert np.isfinite(f).all()
+    assert np.all(np.abs(f[:, idx] - fref) <= TOL * D + 1e-300)
