@@ -174,15 +174,22 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     __syncthreads();
     for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
     __syncthreads();
-#pragma unroll 4
-    for (int j = 0; j < nk; ++j) {
-      const double* row = stage + j * 16;
-      double cpR, hRT, w;
-      thermo_row(row, t, cpR, hRT);
-      tm_ld2(wt + 2 * (k0 + j), w);
+    for (int j0 = 0; j0 < nk; j0 += 4) {  // four accumulators per tensor-memory round trip
+      uint32_t lo[4], hi[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (j0 + u < nk) tm_ld2_raw(wt + 2 * (k0 + j0 + u), lo[u], hi[u]);
       tm_wait_ld();
-      hw = fma(hRT, w, hw);
-      if (store) fout[(size_t)(k0 + j + 1) * ldout] = w * row[0] * irho;
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (j0 + u < nk) {
+          const double* row = stage + (j0 + u) * 16;
+          double cpR, hRT;
+          thermo_row(row, t, cpR, hRT);
+          const double w = __hiloint2double((int)hi[u], (int)lo[u]);
+          hw = fma(hRT, w, hw);
+          if (store) fout[(size_t)(k0 + j0 + u + 1) * ldout] = w * row[0] * irho;
+        }
     }
   }
   if (store) fout[0] = -(t.T * hw) / (rho * cps);
