@@ -44,6 +44,14 @@ __device__ __forceinline__ double thermo_dcp(const MechDev& m, int k, const TSta
   return fma(fma(fma(4.0 * a5, T, 3.0 * a4), T, 2.0 * a3), T, a2);
 }
 
+// Coefficients of the exponential's polynomial (and its reduction constants) in the constant bank: a DFMA takes a
+// constant-bank operand directly, whereas a 64-bit literal costs two UMOV per use inside the hot loops.
+static __constant__ double ck_expc[16] = {
+    0x1.af632a0f7e2cep-26, 0x1.28b4101c77212p-22, 0x1.71ddf56d8deb5p-19, 0x1.a01991a10d9aep-16,
+    0x1.a01a01b1461c5p-13, 0x1.6c16c1880029fp-10, 0x1.111111110f21ep-7,  0x1.555555554f0bap-5,
+    0x1.555555555555ap-3,  0x1.0000000000011p-1,  1.0,                    1.0,
+    1.4426950408889634074, 6755399441055744.0,   -6.93147180369123816490e-01, -1.90821492927058770002e-10};
+
 // exp(x) for the rate constants: x = n ln2 + r, |r| <= ln2/2, degree-11 polynomial (Chebyshev-node interpolation
 // of e^r on [-ln2/2, ln2/2], max relative error 1.6e-17 before rounding), 2^n applied to the exponent field.
 // 15 FP64-pipe instructions + 2 min/max; no branches, no selects: the argument is CLAMPED to [-708, 709], so an
@@ -76,24 +84,15 @@ __device__ __forceinline__ double ck_exp(double x) {
 // The same polynomial without the clamp: ONLY for rows whose arguments the packer has bounded (|x| < 680 over
 // [T_SAFE_LO, T_SAFE_HI]) and temperatures inside that window.  15 FP64-pipe instructions, 3 integer ones.
 __device__ __forceinline__ double ck_exp_nc(double x) {
-  const double MAGIC = 6755399441055744.0;
-  const double t = fma(x, 1.4426950408889634074, MAGIC);
+  const double MAGIC = ck_expc[13];
+  const double t = fma(x, ck_expc[12], MAGIC);
   const int n = __double2loint(t);
   const double nf = t - MAGIC;
-  double r = fma(nf, -6.93147180369123816490e-01, x);
-  r = fma(nf, -1.90821492927058770002e-10, r);
-  double p = 0x1.af632a0f7e2cep-26;
-  p = fma(p, r, 0x1.28b4101c77212p-22);
-  p = fma(p, r, 0x1.71ddf56d8deb5p-19);
-  p = fma(p, r, 0x1.a01991a10d9aep-16);
-  p = fma(p, r, 0x1.a01a01b1461c5p-13);
-  p = fma(p, r, 0x1.6c16c1880029fp-10);
-  p = fma(p, r, 0x1.111111110f21ep-7);
-  p = fma(p, r, 0x1.555555554f0bap-5);
-  p = fma(p, r, 0x1.555555555555ap-3);
-  p = fma(p, r, 0x1.0000000000011p-1);
-  p = fma(p, r, 1.0);
-  p = fma(p, r, 1.0);
+  double r = fma(nf, ck_expc[14], x);
+  r = fma(nf, ck_expc[15], r);
+  double p = ck_expc[0];
+#pragma unroll
+  for (int i = 1; i < 12; ++i) p = fma(p, r, ck_expc[i]);
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 
