@@ -190,8 +190,8 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
       if (WANT_AUX) dci_dM = 1.0;
     } else {
       const double beta0 = xr[1], Ta0 = xr[2];
-      const double k0 = ck_exp(fma(beta0, t.lnT, xr[0]) - Ta0 * t.invT);
-      const double k0_kf = k0 / kf;
+      // k_0 / k_inf from the DIFFERENCE of the two Arrhenius arguments: one exponential, no division
+      const double k0_kf = ck_exp(fma(beta0 - beta, t.lnT, xr[0] - k.lnA) - (Ta0 - Ta) * t.invT);
       const double Pr = k0_kf * M;
       const double inv1p = 1.0 / (1.0 + Pr);
       const double L = Pr * inv1p;  // Lindemann
@@ -209,11 +209,12 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
         const double cc = fma(-0.67, lF, -0.4), nn = fma(-1.27, lF, 0.75);
         const double x = lP + cc;
         const double den = fma(-0.14, x, nn);
-        const double f1 = x / den;
-        const double g = 1.0 / fma(f1, f1, 1.0);
+        const double den2 = den * den;
+        const double g = den2 / fma(x, x, den2);  // 1 / (1 + f1^2), f1 = x / den: one division instead of two
         F = ck_exp(ln10 * lF * g);
         if (WANT_AUX) {
           // ln F = ln10 * lF / (1 + f1^2);  f1 = x/den, x = lP + cc(lF), den = nn(lF) - 0.14 x
+          const double f1 = x / den;
           const double df1_dx = nn / (den * den);              // (den + 0.14 x)/den^2 = nn/den^2
           const double dlnF_df1 = -ln10 * lF * g * g * 2.0 * f1;
           dlnF_dlP = (Pr > 1e-300) ? dlnF_df1 * df1_dx : 0.0;  // d lnF / d log10 Pr
