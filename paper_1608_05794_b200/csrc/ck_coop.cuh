@@ -46,10 +46,13 @@ struct CoopChem {
 };
 struct CoopScalars { double rho, S, cps, Ctot, hw; };
 
-__host__ __device__ inline int coop_chem_doubles(int K, int R, bool jac) {
-  return (K + 1) + 4 * K + R + 40 + (jac ? 12 * R + 3 * K : 0) + 8;
+// jc > 0: the per-reaction derivative arrays hold one CHUNK of jc reactions (rhs_jac_coop); jc = 0: all R reactions
+__host__ __device__ inline int coop_chem_doubles(int K, int R, bool jac, int jc = 0) {
+  const int L = jc > 0 ? jc : R;
+  return (K + 1) + 4 * K + R + 40 + (jac ? 12 * L + 3 * K : 0) + 8;
 }
-__device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool jac) {
+__device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool jac, int jc = 0) {
+  const int L = jc > 0 ? jc : R;
   CoopChem c;
   c.C = base; base += K + 1;
   c.cpR = base; base += K;
@@ -58,10 +61,10 @@ __device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool 
   c.w = base; base += K;
   c.q = base; base += R;
   c.red = base; base += 40;
-  c.dqs = base; base += jac ? 6 * R : 0;
-  c.dqT = base; base += jac ? R : 0;
-  c.dqM = base; base += jac ? R : 0;
-  c.si = base; base += jac ? R : 0;
+  c.dqs = base; base += jac ? 6 * L : 0;
+  c.dqT = base; base += jac ? L : 0;
+  c.dqM = base; base += jac ? L : 0;
+  c.si = base; base += jac ? L : 0;
   c.dns = base; base += jac ? K : 0;
   c.sig = base; base += jac ? K : 0;
   c.tau = base; base += jac ? K : 0;
@@ -145,12 +148,176 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
   return s;
 }
 
+// f(y) AND the species rows G_kj of the analytic Jacobian in one pass over the reactions, G reactions at a time:
+// the per-reaction derivative arrays then hold a single chunk (12 G doubles instead of 12 R), which is what lets
+// more reactors share an SM.  Requires K <= G (thread k owns species row k and walks its reaction list, sorted by
+// reaction index, with a private cursor).  Leaves q, omega, f, dns / sig / tau as rhs_coop<.,true> + the row phase
+// of jac_coop would; the caller finishes with jac_coop_finish.  A is zeroed here.
+template <int G>
+__device__ __forceinline__ CoopScalars rhs_jac_coop(const MechDev& m, const double* __restrict__ y, double p,
+                                                    double* __restrict__ fout, const CoopChem& c, TState& t,
+                                                    double* __restrict__ A, int lda) {
+  const int K = m.K, R = m.R, N = K + 1, tid = threadIdx.x;
+  t = make_tstate(m, y[0]);
+  double Sp = 0.0, cp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    double cpR, hRT;
+    thermo_cp_h(m, k, t, cpR, hRT);
+    const double yw = y[1 + k] * __ldg(m.invW + k);
+    c.cpR[k] = cpR; c.hRT[k] = hRT; c.yw[k] = yw;
+    Sp += yw;
+    cp = fma(yw, cpR, cp);
+  }
+  for (int idx = tid; idx < N * lda; idx += G) A[idx] = 0.0;
+  CoopScalars s;
+  s.S = block_sum<G>(Sp, c.red);
+  s.cps = block_sum<G>(cp, c.red);
+  s.Ctot = p / (R_U * t.T);
+  s.rho = s.Ctot / s.S;
+  for (int k = tid; k < K; k += G) c.C[k] = s.rho * c.yw[k];
+  if (tid == 0) c.C[K] = 1.0;
+  __syncthreads();
+  const bool has_row = tid < K;
+  double* row = A + (size_t)(1 + (has_row ? tid : 0)) * lda + 1;
+  int e = has_row ? __ldg(m.tptr + tid) : 0;
+  const int e1 = has_row ? __ldg(m.tptr + tid + 1) : 0;
+  double dns = 0.0, sig = 0.0, tau = 0.0;
+  for (int c0 = 0; c0 < R; c0 += G) {
+    const int r = c0 + tid;
+    if (r < R) {
+      const RxnConst kc = load_rxn_global(m, r, t.tint);
+      RateAux a;
+      const double q = reaction_q<1, true>(m, r, kc, t, c.C, s.Ctot, &a);
+      c.q[r] = q;
+      const double x0 = c.C[kc.slot[0]], x1 = c.C[kc.slot[1]], x2 = c.C[kc.slot[2]];
+      const double x3 = c.C[kc.slot[3]], x4 = c.C[kc.slot[4]], x5 = c.C[kc.slot[5]];
+      const double gf = a.ci * a.kf, gr = -a.ci * a.kr;
+      double d[6] = {gf * x1 * x2, gf * x0 * x2, gf * x0 * x1, gr * x4 * x5, gr * x3 * x5, gr * x3 * x4};
+      double sum = 0.0;
+#pragma unroll
+      for (int x = 0; x < 6; ++x) {
+        if (kc.slot[x] == K) d[x] = 0.0;
+        c.dqs[x * G + tid] = d[x];
+        c.dsl[x * G + tid] = kc.slot[x];
+        sum = fma(d[x], c.C[kc.slot[x]], sum);
+      }
+      const double net = a.kf * a.pf - a.kr * a.pr;
+      const double dM = a.dci_dM * net;
+      c.dqM[tid] = dM;
+      c.dqT[tid] = a.ci * (a.kf * a.pf * a.dlnkf_dT - a.kr * a.pr * a.dlnkr_dT) + a.dci_dT * net;
+      double M = 0.0;
+      if (r >= m.r_tb) {
+        const int j = r - m.r_tb;
+        M = s.Ctot;
+        for (int z = __ldg(m.eptr + j), z1 = __ldg(m.eptr + j + 1); z < z1; ++z)
+          M = fma(__ldg(m.eval1 + z), c.C[__ldg(m.espec + z)], M);
+      }
+      c.si[tid] = fma(dM, M, sum);
+    }
+    __syncthreads();
+    // species rows: entries of this chunk (the reaction list of a row is sorted by reaction index)
+    while (e < e1) {
+      const int en = __ldg(m.tent + e);
+      const int i = en >> 8;
+      if (i >= c0 + G) break;
+      const int j = i - c0;
+      const double nu = (double)((en & 255) - 128);
+      int sl[6];
+      double d[6], rv[6];
+#pragma unroll
+      for (int x = 0; x < 6; ++x) { sl[x] = c.dsl[x * G + j]; d[x] = c.dqs[x * G + j]; }
+#pragma unroll
+      for (int x = 1; x < 6; ++x)
+#pragma unroll
+        for (int y2 = 0; y2 < x; ++y2)
+          if (sl[x] == sl[y2] && sl[x] != K) { d[y2] += d[x]; sl[x] = K; }
+#pragma unroll
+      for (int x = 0; x < 6; ++x)
+        if (sl[x] != K) rv[x] = row[sl[x]];
+#pragma unroll
+      for (int x = 0; x < 6; ++x)
+        if (sl[x] != K) row[sl[x]] = fma(nu, d[x], rv[x]);
+      sig = fma(nu, c.si[j], sig);
+      tau = fma(nu, c.dqT[j], tau);
+      if (i >= m.r_tb) {
+        const double dM = nu * c.dqM[j];
+        dns += dM;
+        const int jj = i - m.r_tb;
+        for (int z = __ldg(m.eptr + jj), z1 = __ldg(m.eptr + jj + 1); z < z1; ++z) {
+          const int sp = __ldg(m.espec + z);
+          row[sp] = fma(dM, __ldg(m.eval1 + z), row[sp]);
+        }
+      }
+      ++e;
+    }
+    __syncthreads();
+  }
+  if (has_row) { c.dns[tid] = dns; c.sig[tid] = sig; c.tau[tid] = tau; }
+  const double irho = 1.0 / s.rho;
+  double hwp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    double w = 0.0;
+    for (int z = __ldg(m.tptr + k), z1 = __ldg(m.tptr + k + 1); z < z1; ++z) {
+      const int en = __ldg(m.tent + z);
+      w = fma((double)((en & 255) - 128), c.q[en >> 8], w);
+    }
+    c.w[k] = w;
+    hwp = fma(c.hRT[k], w, hwp);
+    fout[1 + k] = w * __ldg(m.W + k) * irho;
+  }
+  s.hw = block_sum<G>(hwp, c.red);
+  if (tid == 0) fout[0] = -(t.T * s.hw) / (s.rho * s.cps);
+  __syncthreads();
+  return s;
+}
+
 // Analytic Jacobian A[i*lda + j] = d f_i / d y_j (i, j = 0 is T) from the pieces left in shared memory by
 // rhs_coop<G,true>; `f` is that call's output.  Chain rule at constant p:
 //   C_m = rho Y_m / W_m, rho = p/(R_u T S):  dC_m/dT = -C_m/T,  dC_m/dY_j = delta_mj rho/W_j - C_m/(S W_j)
 //   G_kj = sum_i nu_ki dq_i/dC_j,  sigma_k = sum_i nu_ki sum_m dq_i/dC_m C_m,  tau_k = sum_i nu_ki dq_i/dT|_C
 //   d omega_k/dY_j = (rho/W_j) G_kj - sigma_k/(S W_j),   d omega_k/dT = tau_k - sigma_k/T
 // Ends with a __syncthreads().
+// temperature row, temperature column and the in-place transform of the species block (see jac_coop)
+template <int G>
+__device__ __forceinline__ void jac_coop_finish(const MechDev& m, const CoopChem& c, const CoopScalars& s, const TState& t,
+                                         const double* __restrict__ f, double* __restrict__ A, int lda) {
+  const int K = m.K, tid = threadIdx.x;
+  // scalars of the temperature row
+  double hs = 0.0, ht = 0.0, hcw = 0.0, dcp = 0.0;
+  for (int k = tid; k < K; k += G) {
+    hs = fma(c.hRT[k], c.sig[k], hs);
+    ht = fma(c.hRT[k], c.tau[k] - c.sig[k] * t.invT, ht);
+    hcw = fma((c.cpR[k] - c.hRT[k]) * t.invT, c.w[k], hcw);
+    dcp = fma(c.yw[k], thermo_dcp(m, k, t), dcp);
+  }
+  hs = block_sum<G>(hs, c.red);
+  ht = block_sum<G>(ht, c.red);
+  hcw = block_sum<G>(hcw, c.red);
+  dcp = block_sum<G>(dcp, c.red);
+  const double phi = t.T / (s.rho * s.cps);
+  const double fT = f[0];
+  const double iS = 1.0 / s.S;
+  for (int j = tid; j < K; j += G) {
+    double col = 0.0;
+    for (int k = 0; k < K; ++k) col = fma(c.hRT[k], A[(size_t)(1 + k) * lda + 1 + j] + c.dns[k], col);
+    const double iWj = __ldg(m.invW + j);
+    A[1 + j] = -phi * (s.rho * iWj * col - hs * iS * iWj) + fT * (iS * iWj - c.cpR[j] * iWj / s.cps);
+  }
+  if (tid == 0) A[0] = -phi * (hcw + ht) + fT * (2.0 * t.invT - dcp / s.cps);
+  __syncthreads();
+  // species rows: in-place transform of G into d f_k / d Y_j, and the temperature column
+  const double irho = 1.0 / s.rho;
+  for (int idx = tid; idx < K * K; idx += G) {
+    const int k = idx / K, j = idx - k * K;
+    const double Wk = __ldg(m.W + k), iWj = __ldg(m.invW + j);
+    double* a = A + (size_t)(1 + k) * lda + 1 + j;
+    *a = Wk * iWj * (*a + c.dns[k]) + (f[1 + k] - Wk * irho * c.sig[k]) * iS * iWj;
+  }
+  for (int k = tid; k < K; k += G)
+    A[(size_t)(1 + k) * lda] = __ldg(m.W + k) * irho * (c.tau[k] - c.sig[k] * t.invT) + f[1 + k] * t.invT;
+  __syncthreads();
+}
+
 template <int G>
 __device__ __forceinline__ void jac_coop(const MechDev& m, const CoopChem& c, const CoopScalars& s, const TState& t,
                                          const double* __restrict__ f, double* __restrict__ A, int lda) {
@@ -197,40 +364,7 @@ __device__ __forceinline__ void jac_coop(const MechDev& m, const CoopChem& c, co
     c.dns[k] = dns; c.sig[k] = sig; c.tau[k] = tau;
   }
   __syncthreads();
-  // scalars of the temperature row
-  double hs = 0.0, ht = 0.0, hcw = 0.0, dcp = 0.0;
-  for (int k = tid; k < K; k += G) {
-    hs = fma(c.hRT[k], c.sig[k], hs);
-    ht = fma(c.hRT[k], c.tau[k] - c.sig[k] * t.invT, ht);
-    hcw = fma((c.cpR[k] - c.hRT[k]) * t.invT, c.w[k], hcw);
-    dcp = fma(c.yw[k], thermo_dcp(m, k, t), dcp);
-  }
-  hs = block_sum<G>(hs, c.red);
-  ht = block_sum<G>(ht, c.red);
-  hcw = block_sum<G>(hcw, c.red);
-  dcp = block_sum<G>(dcp, c.red);
-  const double phi = t.T / (s.rho * s.cps);
-  const double fT = f[0];
-  const double iS = 1.0 / s.S;
-  for (int j = tid; j < K; j += G) {
-    double col = 0.0;
-    for (int k = 0; k < K; ++k) col = fma(c.hRT[k], A[(size_t)(1 + k) * lda + 1 + j] + c.dns[k], col);
-    const double iWj = __ldg(m.invW + j);
-    A[1 + j] = -phi * (s.rho * iWj * col - hs * iS * iWj) + fT * (iS * iWj - c.cpR[j] * iWj / s.cps);
-  }
-  if (tid == 0) A[0] = -phi * (hcw + ht) + fT * (2.0 * t.invT - dcp / s.cps);
-  __syncthreads();
-  // species rows: in-place transform of G into d f_k / d Y_j, and the temperature column
-  const double irho = 1.0 / s.rho;
-  for (int idx = tid; idx < K * K; idx += G) {
-    const int k = idx / K, j = idx - k * K;
-    const double Wk = __ldg(m.W + k), iWj = __ldg(m.invW + j);
-    double* a = A + (size_t)(1 + k) * lda + 1 + j;
-    *a = Wk * iWj * (*a + c.dns[k]) + (f[1 + k] - Wk * irho * c.sig[k]) * iS * iWj;
-  }
-  for (int k = tid; k < K; k += G)
-    A[(size_t)(1 + k) * lda] = __ldg(m.W + k) * irho * (c.tau[k] - c.sig[k] * t.invT) + f[1 + k] * t.invT;
-  __syncthreads();
+  jac_coop_finish<G>(m, c, s, t, f, A, lda);
 }
 
 }  // namespace ck

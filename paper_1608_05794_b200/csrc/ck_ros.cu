@@ -30,9 +30,11 @@ constexpr double e1 = -0.2815431932141155, e2 = -0.07276199124938920, e3 = -0.10
 
 __host__ __device__ inline int ros_lda(int N) { return N | 1; }
 // doubles of dynamic shared memory of the ROS4 / jac kernels
-__host__ __device__ inline size_t ros_smem_doubles(int K, int R) {
+// chunk length of the per-reaction derivative arrays: G when thread k can own species row k, else all reactions
+__host__ __device__ inline int ros_jc(int K, int G) { return K <= G ? G : 0; }
+__host__ __device__ inline size_t ros_smem_doubles(int K, int R, int G) {
   const int N = K + 1;
-  return (size_t)N * ros_lda(N) + 12 * (size_t)N + (size_t)(N + 1) / 2 + 8 + coop_chem_doubles(K, R, true);
+  return (size_t)N * ros_lda(N) + 12 * (size_t)N + (size_t)(N + 1) / 2 + 8 + coop_chem_doubles(K, R, true, ros_jc(K, G));
 }
 
 struct RosShared {
@@ -40,7 +42,7 @@ struct RosShared {
   int* piv;
   CoopChem c;
 };
-__device__ __forceinline__ RosShared ros_carve(double* sm, int K, int R) {
+__device__ __forceinline__ RosShared ros_carve(double* sm, int K, int R, int G) {
   const int N = K + 1;
   RosShared s;
   s.A = sm; sm += (size_t)N * ros_lda(N);
@@ -48,7 +50,7 @@ __device__ __forceinline__ RosShared ros_carve(double* sm, int K, int R) {
   s.u1 = sm; sm += N; s.u2 = sm; sm += N; s.u3 = sm; sm += N; s.u4 = sm; sm += N;
   s.yt = sm; sm += N; s.rhs = sm; sm += N; s.tmp = sm; sm += N; s.e = sm; sm += N;
   s.piv = reinterpret_cast<int*>(sm); sm += (N + 1) / 2 + 8;
-  s.c = coop_carve(sm, K, R, true);
+  s.c = coop_carve(sm, K, R, true, ros_jc(K, G));
   return s;
 }
 
@@ -69,9 +71,15 @@ __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, dou
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   TState t;
   if (mode == CK_JAC_ANALYTIC) {
-    const CoopScalars sc = rhs_coop<G, true>(m, s.y, p, s.f0, s.c, t);
-    if (clk_mid) *clk_mid = clock64();
-    jac_coop<G>(m, s.c, sc, t, s.f0, s.A, lda);
+    if (m.K <= G) {  // one pass over the reactions, derivative arrays one chunk long
+      const CoopScalars sc = rhs_jac_coop<G>(m, s.y, p, s.f0, s.c, t, s.A, lda);
+      if (clk_mid) *clk_mid = clock64();
+      jac_coop_finish<G>(m, s.c, sc, t, s.f0, s.A, lda);
+    } else {
+      const CoopScalars sc = rhs_coop<G, true>(m, s.y, p, s.f0, s.c, t);
+      if (clk_mid) *clk_mid = clock64();
+      jac_coop<G>(m, s.c, sc, t, s.f0, s.A, lda);
+    }
     return 1;
   }
   if (clk_mid) *clk_mid = clock64();
@@ -100,7 +108,7 @@ __global__ void __launch_bounds__(G) jac_kernel(const MechDev m, long long n, co
                                                 const double* __restrict__ p, int mode, double h, double rtol, double atol,
                                                 double* __restrict__ J, long long ldJ) {
   extern __shared__ double sm[];
-  RosShared s = ros_carve(sm, m.K, m.R);
+  RosShared s = ros_carve(sm, m.K, m.R, G);
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   for (long long r = blockIdx.x; r < n; r += gridDim.x) {
     __syncthreads();
@@ -172,7 +180,7 @@ __global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs 
   using namespace ros4c;
   extern __shared__ double sm[];
   __shared__ long long s_next;
-  RosShared s = ros_carve(sm, m.K, m.R);
+  RosShared s = ros_carve(sm, m.K, m.R, G);
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   long long c_att = 0, c_acc = 0, c_rej = 0, c_rhs = 0, c_jac = 0, c_fail = 0;
   long long ck[7] = {0, 0, 0, 0, 0, 0, 0};
@@ -345,7 +353,7 @@ constexpr size_t SMEM_CAP = 227 * 1024;
 template <int G>
 int32_t launch_jac(const ck_mech* m, long long n, const double* y, long long ld, const double* p, int mode, double h,
                    double rtol, double atol, double* J, long long ldJ, cudaStream_t st) {
-  const size_t smem = ros_smem_doubles(m->K, m->R) * sizeof(double);
+  const size_t smem = ros_smem_doubles(m->K, m->R, G) * sizeof(double);
   CK_CUDA(cudaFuncSetAttribute(jac_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0, sms = 0;
   CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, jac_kernel<G>, G, smem));
@@ -358,7 +366,7 @@ int32_t launch_jac(const ck_mech* m, long long n, const double* y, long long ld,
 
 template <int G, int NR, int NS>
 int32_t launch_ros(const ck_mech* m, const RosArgs& a, int* grid_out, cudaStream_t st) {
-  const size_t smem = ros_smem_doubles(m->K, m->R) * sizeof(double);
+  const size_t smem = ros_smem_doubles(m->K, m->R, G) * sizeof(double);
   CK_CUDA(cudaFuncSetAttribute(ros4_kernel<G, NR, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0, sms = 0;
   CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros4_kernel<G, NR, NS>, G, smem));
@@ -379,7 +387,7 @@ extern "C" int32_t ck_jac(const ck_mech* m, int64_t n, const double* y, int64_t 
   if (n == 0) return CK_OK;
   if (!y || !p || !J) { set_error("ck_jac: null batch pointer"); return CK_EINVAL; }
   const int N = m->K + 1;
-  if (ros_smem_doubles(m->K, m->R) * sizeof(double) > SMEM_CAP) { set_error("ck_jac: %d x %d matrix does not fit shared memory", N, N); return CK_EUNSUPPORTED; }
+  if (ros_smem_doubles(m->K, m->R, group_size(N)) * sizeof(double) > SMEM_CAP) { set_error("ck_jac: %d x %d matrix does not fit shared memory", N, N); return CK_EUNSUPPORTED; }
   CK_CUDA(cudaSetDevice(m->device));
   cudaStream_t st = (cudaStream_t)stream;
   switch (group_size(N)) {
@@ -437,7 +445,7 @@ extern "C" int32_t ck_integrate_ros(const ck_mech* m, int64_t n, double* y, int6
   if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
   if (o->jac_mode != CK_JAC_ANALYTIC && o->jac_mode != CK_JAC_FD) { set_error("ck_integrate_ros: bad jac_mode"); return CK_EINVAL; }
   const int N = m->K + 1;
-  if (ros_smem_doubles(m->K, m->R) * sizeof(double) > SMEM_CAP || N > 256) { set_error("ck_integrate_ros: %d x %d matrix does not fit shared memory", N, N); return CK_EUNSUPPORTED; }
+  if (ros_smem_doubles(m->K, m->R, group_size(N)) * sizeof(double) > SMEM_CAP || N > 256) { set_error("ck_integrate_ros: %d x %d matrix does not fit shared memory", N, N); return CK_EUNSUPPORTED; }
   RosArgs a;
   a.n = n; a.ld = ld; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
   a.jac_mode = o->jac_mode; a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.use_queue = !(o->flags & 1);
