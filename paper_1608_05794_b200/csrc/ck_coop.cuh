@@ -194,13 +194,24 @@ __device__ __forceinline__ CoopScalars rhs_jac_coop(const MechDev& m, const doub
       const double gf = a.ci * a.kf, gr = -a.ci * a.kr;
       double d[6] = {gf * x1 * x2, gf * x0 * x2, gf * x0 * x1, gr * x4 * x5, gr * x3 * x5, gr * x3 * x4};
       double sum = 0.0;
+      int sl[6];
 #pragma unroll
       for (int x = 0; x < 6; ++x) {
-        if (kc.slot[x] == K) d[x] = 0.0;
-        c.dqs[x * G + tid] = d[x];
-        c.dsl[x * G + tid] = kc.slot[x];
-        sum = fma(d[x], c.C[kc.slot[x]], sum);
+        sl[x] = kc.slot[x];
+        if (sl[x] == K) d[x] = 0.0;
+        sum = fma(d[x], c.C[sl[x]], sum);
       }
+      // a species may sit in two slots (nu = 2, or on both sides): fold the later slot into the earlier one HERE,
+      // once per reaction, so that the row assembly can load, update and store a reaction's entries together
+      if (__ldg(m.rflag + r)) {
+#pragma unroll
+        for (int x = 1; x < 6; ++x)
+#pragma unroll
+          for (int y2 = 0; y2 < x; ++y2)
+            if (sl[x] == sl[y2] && sl[x] != K) { d[y2] += d[x]; d[x] = 0.0; sl[x] = K; }
+      }
+#pragma unroll
+      for (int x = 0; x < 6; ++x) { c.dqs[x * G + tid] = d[x]; c.dsl[x * G + tid] = sl[x]; }
       const double net = a.kf * a.pf - a.kr * a.pr;
       const double dM = a.dci_dM * net;
       c.dqM[tid] = dM;
@@ -226,11 +237,6 @@ __device__ __forceinline__ CoopScalars rhs_jac_coop(const MechDev& m, const doub
       double d[6], rv[6];
 #pragma unroll
       for (int x = 0; x < 6; ++x) { sl[x] = c.dsl[x * G + j]; d[x] = c.dqs[x * G + j]; }
-#pragma unroll
-      for (int x = 1; x < 6; ++x)
-#pragma unroll
-        for (int y2 = 0; y2 < x; ++y2)
-          if (sl[x] == sl[y2] && sl[x] != K) { d[y2] += d[x]; sl[x] = K; }
 #pragma unroll
       for (int x = 0; x < 6; ++x)
         if (sl[x] != K) rv[x] = row[sl[x]];

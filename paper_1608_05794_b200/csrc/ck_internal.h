@@ -40,6 +40,7 @@ struct MechDev {
   const double* Ta;           // [R]  Ea / R_cal
   const double* krc;          // [nT][7][R]  ln k_r = c0 + c1 lnT + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4
   const int* slot;            // [6][R]  slots 0-2 reactants, 3-5 products (species index or K)
+  const int* rflag;           // [R]  bit 0: a species sits in two slots of the reaction
   const double* rpack;        // [R][rstride] AoS for smem staging: lnA, beta, Ta, slots (6 x 10 bit in the
                               //   low/high 32-bit words), then per interval 8 doubles: c0..c6, 0
   int rstride;                // = 4 + 8 nT

@@ -241,6 +241,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   if (K > 1022) { set_error("ck_mech_load: more than 1022 species"); return CK_EUNSUPPORTED; }
   const int rstride = 4 + 8 * nT;
   std::vector<double> rpack((size_t)std::max(R, 1) * rstride, 0.0);
+  std::vector<int> rflag(std::max(R, 1), 0);
   for (int r = 0; r < R; ++r) {
     double* q = &rpack[(size_t)r * rstride];
     q[0] = lnA[r]; q[1] = beta[r]; q[2] = Ta[r];
@@ -250,7 +251,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     for (int s = 0; s < 6; ++s)
       for (int s2 = 0; s2 < s; ++s2)
         if (slot[(size_t)s * R + r] != K && slot[(size_t)s * R + r] == slot[(size_t)s2 * R + r]) dup = true;
-    if (dup) w[1] |= 0x80000000u;
+    if (dup) { w[1] |= 0x80000000u; rflag[r] = 1; }
     std::memcpy(&q[3], w, sizeof w);
     for (int t = 0; t < nT; ++t)
       for (int j = 0; j < 7; ++j) q[4 + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];
@@ -283,7 +284,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   // ---- arena + upload -------------------------------------------------------------------------------
   Arena a;
   size_t oW = a.put(W), oiW = a.put(invW), olo = a.put(nlo), ohi = a.put(nhi), otm = a.put(tmid);
-  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), oslot = a.put(slot), osp = a.put(spack), oxp = a.put(xpack);
+  size_t olnA = a.put(lnA), ob = a.put(beta), oTa = a.put(Ta), okrc = a.put(krc), oslot = a.put(slot), osp = a.put(spack), oxp = a.put(xpack), orf = a.put(rflag);
   size_t oep = a.put(eptr), oes = a.put(espec), oev = a.put(eval1);
   size_t olnA0 = a.put(lnA0), ob0 = a.put(beta0), oTa0 = a.put(Ta0), otroe = a.put(troe);
   size_t otp = a.put(tptr), ote = a.put(tent), operm = a.put(perm), orp = a.put(rpack);
@@ -308,7 +309,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);
   v.nlo = (const double*)(base + olo); v.nhi = (const double*)(base + ohi); v.tmid = (const double*)(base + otm);
   v.lnA = (const double*)(base + olnA); v.beta = (const double*)(base + ob); v.Ta = (const double*)(base + oTa);
-  v.krc = (const double*)(base + okrc); v.slot = (const int*)(base + oslot); v.spack = (const double*)(base + osp); v.xpack = (const double*)(base + oxp);
+  v.krc = (const double*)(base + okrc); v.slot = (const int*)(base + oslot); v.spack = (const double*)(base + osp); v.xpack = (const double*)(base + oxp); v.rflag = (const int*)(base + orf);
   v.eptr = (const int*)(base + oep); v.espec = (const int*)(base + oes); v.eval1 = (const double*)(base + oev);
   v.lnA0 = (const double*)(base + olnA0); v.beta0 = (const double*)(base + ob0); v.Ta0 = (const double*)(base + oTa0);
   v.troe = (const double*)(base + otroe);

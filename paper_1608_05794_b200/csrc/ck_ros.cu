@@ -175,8 +175,12 @@ __device__ __forceinline__ void solve_rows_smem(const double* __restrict__ A, in
   __syncthreads();
 }
 
+// minimum resident CTAs per SM the register allocation must allow (shared memory sets the real limit:
+// 5 at N = 54; without the bound the kernel takes 254 registers and only 4 CTAs of 64 threads fit)
+constexpr int ros_min_ctas(int G) { return G == 32 ? 12 : (G == 64 ? 5 : 1); }
+
 template <int G, int NR, int NS>
-__global__ void __launch_bounds__(G) ros4_kernel(const MechDev m, const RosArgs a) {
+__global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const MechDev m, const RosArgs a) {
   using namespace ros4c;
   extern __shared__ double sm[];
   __shared__ long long s_next;
@@ -372,6 +376,7 @@ int32_t launch_ros(const ck_mech* m, const RosArgs& a, int* grid_out, cudaStream
   CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros4_kernel<G, NR, NS>, G, smem));
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
   const long long grid = std::min<long long>(a.n, (long long)std::max(per_sm, 1) * sms);
+  if (getenv("CK_DEBUG")) fprintf(stderr, "ros4_kernel<%d,%d,%d>: smem %zu B, %d CTAs/SM, grid %lld\n", G, NR, NS, smem, per_sm, grid);
   ros4_kernel<G, NR, NS><<<(unsigned)grid, G, smem, st>>>(m->dev, a);
   CK_CUDA(cudaGetLastError());
   *grid_out = (int)grid;
