@@ -96,6 +96,45 @@ __device__ __forceinline__ double ck_exp_nc(double x) {
   return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));
 }
 
+// 1/y and ln(x) for the falloff rows: branch-free, a few ulp (the library versions are correctly rounded but cost
+// ~22 and ~65 instructions with a slow-path branch each; a Troe row needs two logarithms and two divisions).
+__device__ __forceinline__ double ck_rcp(double y) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(y));   // ~20 good bits
+  double e = fma(-y, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-y, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-y, r, 1.0);
+  return fma(r, e, r);
+}
+// x must be a positive NORMAL number (callers guard with fmax(x, 1e-300))
+__device__ __forceinline__ double ck_log(double x) {
+  int hi = __double2hiint(x);
+  int e = (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;                    // mantissa in [1, 2)
+  double mnt = __hiloint2double(hi, __double2loint(x));
+  const bool big = mnt > 1.4142135623730951;
+  mnt = big ? mnt * 0.5 : mnt;                            // [sqrt(1/2), sqrt(2)]
+  e += big ? 1 : 0;
+  const double f = mnt - 1.0;
+  const double s = f * ck_rcp(2.0 + f);                   // ln(m) = 2 atanh(s), |s| <= 0.1716
+  const double z = s * s;
+  double p = 1.0 / 21.0;
+  p = fma(p, z, 1.0 / 19.0);
+  p = fma(p, z, 1.0 / 17.0);
+  p = fma(p, z, 1.0 / 15.0);
+  p = fma(p, z, 1.0 / 13.0);
+  p = fma(p, z, 1.0 / 11.0);
+  p = fma(p, z, 1.0 / 9.0);
+  p = fma(p, z, 1.0 / 7.0);
+  p = fma(p, z, 1.0 / 5.0);
+  p = fma(p, z, 1.0 / 3.0);
+  const double lm = fma(2.0 * s * z, p, 2.0 * s);
+  const double ed = (double)e;
+  return fma(ed, 6.93147180369123816490e-01, fma(ed, 1.90821492927058770002e-10, lm));
+}
+
 // Constants of one reaction gathered into registers (from the SoA arrays or from a staged rpack row).
 struct RxnConst {
   double lnA, beta, Ta, c0, c1, c2, c3, c4, c5, c6;
@@ -193,7 +232,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
       // k_0 / k_inf from the DIFFERENCE of the two Arrhenius arguments: one exponential, no division
       const double k0_kf = ck_exp(fma(beta0 - beta, t.lnT, xr[0] - k.lnA) - (Ta0 - Ta) * t.invT);
       const double Pr = k0_kf * M;
-      const double inv1p = 1.0 / (1.0 + Pr);
+      const double inv1p = ck_rcp(1.0 + Pr);
       const double L = Pr * inv1p;  // Lindemann
       double F = 1.0, dlnF_dlP = 0.0, dlnF_dT = 0.0;
       if (r >= m.r_troe) {
@@ -205,12 +244,12 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
         const double il10 = 0.43429448190325182765;  // 1/ln 10
         const double ln10 = 2.30258509299404568402;
         const double Fcg = fmax(Fc, 1e-300), Prg = fmax(Pr, 1e-300);
-        const double lF = log(Fcg) * il10, lP = log(Prg) * il10;
+        const double lF = ck_log(Fcg) * il10, lP = ck_log(Prg) * il10;
         const double cc = fma(-0.67, lF, -0.4), nn = fma(-1.27, lF, 0.75);
         const double x = lP + cc;
         const double den = fma(-0.14, x, nn);
         const double den2 = den * den;
-        const double g = den2 / fma(x, x, den2);  // 1 / (1 + f1^2), f1 = x / den: one division instead of two
+        const double g = den2 * ck_rcp(fma(x, x, den2));  // 1 / (1 + f1^2), f1 = x / den: one reciprocal instead of two divisions
         F = ck_exp(ln10 * lF * g);
         if (WANT_AUX) {
           // ln F = ln10 * lF / (1 + f1^2);  f1 = x/den, x = lP + cc(lF), den = nn(lF) - 0.14 x

@@ -27,6 +27,7 @@ struct MechDev {
   int K, R, nT;
   int r_22;                   // leading rows of the plain group that are A + B <=> C + D with four distinct species
   int r_dup, r_tb, r_lind, r_troe;
+  int r_tbf;                  // [r_tb, r_tbf): three-body rows with distinct slot species, bounded exponents, <= 6 efficiencies
   double t_safe_lo, t_safe_hi;  // see ck_mech.cu `bounded`
   double tedge[MAX_TINT];     // interval t holds tedge[t-1] < T <= tedge[t]; nT-1 finite edges
   const double* W;            // [K]

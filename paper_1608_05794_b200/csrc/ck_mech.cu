@@ -141,7 +141,14 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   for (int i = 0; i < R; ++i) if (!slow[i] && is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; r_22++; }
   for (int i = 0; i < R; ++i) if (!slow[i] && !is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
   for (int i = 0; i < R; ++i) if (d->type[i] == 0 && slow[i]) { perm.push_back(i); cnt[0]++; }
-  for (int t = 1; t < 4; ++t)
+  int n_tbf = 0;  // three-body rows that qualify for the fast path come first in their group
+  auto tb_fast = [&](int i) {
+    return d->type[i] == 1 && d->eff_ptr && !has_dup(i) && bounded(i) && d->eff_ptr[i + 1] - d->eff_ptr[i] <= 6 &&
+           d->eff_ptr[i + 1] >= d->eff_ptr[i];
+  };
+  for (int i = 0; i < R; ++i) if (tb_fast(i)) { perm.push_back(i); cnt[1]++; n_tbf++; }
+  for (int i = 0; i < R; ++i) if (d->type[i] == 1 && !tb_fast(i)) { perm.push_back(i); cnt[1]++; }
+  for (int t = 2; t < 4; ++t)
     for (int i = 0; i < R; ++i)
       if (d->type[i] == t) { perm.push_back(i); cnt[t]++; }
   const int r_tb = cnt[0], r_lind = cnt[0] + cnt[1], r_troe = r_lind + cnt[2];
@@ -304,6 +311,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   MechDev& v = m->dev;
   v.K = K; v.R = R; v.nT = nT;
   v.t_safe_lo = T_SAFE_LO; v.t_safe_hi = T_SAFE_HI;
+  v.r_tbf = r_tb + n_tbf;
   v.r_22 = r_22; v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
   for (int t = 0; t < MAX_TINT; ++t) v.tedge[t] = (t < nT - 1) ? edges[t] : std::numeric_limits<double>::infinity();
   v.W = (const double*)(base + oW); v.invW = (const double*)(base + oiW);
@@ -329,6 +337,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   }
   m->K = K; m->R = R; m->n_tb = cnt[1]; m->n_lind = cnt[2]; m->n_troe = cnt[3]; m->n_rev = n_rev;
   m->n_part = n_part; m->n_eff = (long long)espec.size();
+  if (getenv("CK_DEBUG")) fprintf(stderr, "ck_mech_load: K=%d R=%d groups: r_22=%d r_dup=%d r_tb=%d r_lind=%d r_troe=%d r_tbf=%d nT=%d\n", K, R, v.r_22, v.r_dup, v.r_tb, v.r_lind, v.r_troe, v.r_tbf, nT);
   *out = m;
   return CK_OK;
 }
