@@ -54,13 +54,18 @@ static __constant__ double ck_expc[16] = {
 
 // exp(x) for the rate constants: x = n ln2 + r, |r| <= ln2/2, degree-11 polynomial (Chebyshev-node interpolation
 // of e^r on [-ln2/2, ln2/2], max relative error 1.6e-17 before rounding), 2^n applied to the exponent field.
-// 15 FP64-pipe instructions + 2 min/max; no branches, no selects: the argument is CLAMPED to [-708, 709], so an
+// 15 FP64-pipe instructions; no branches: the argument is CLAMPED to [-708, 708], so an
 // irreversible reaction (c0 = -inf) gets k_r = 3e-308 instead of 0 (absolute effect < 1e-300 on any rate) and
 // an overflowing argument saturates at 8e307.  With 16 warps per SM the Horner chain is hidden by other warps
 // (an Estrin form, 4 more instructions, was faster only at 8 warps per SM).
 __device__ __forceinline__ double ck_exp(double x) {
   const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52
-  x = fmin(fmax(x, -708.0), 709.0);
+  {  // clamp |x| to 708 with integer operations on the high word (FP64 min/max is a DSETP + two selects each, on
+     // the contended FP64 pipe); NaN and infinities land on +-708 as well
+    const int hx = __double2hiint(x);
+    const bool big = (hx & 0x7fffffff) >= 0x40862000;
+    x = big ? __hiloint2double((hx & 0x80000000) | 0x40862000, 0) : x;
+  }
   const double t = fma(x, 1.4426950408889634074, MAGIC);
   const int n = __double2loint(t);
   const double nf = t - MAGIC;
