@@ -14,6 +14,7 @@ constexpr double R_U = 8.31446261815324e7;  // erg/(mol K)
 constexpr double R_CAL = 1.98720425864083;  // cal/(mol K)
 constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere")
 constexpr int MAX_TINT = 8;
+constexpr int SPS = 28;  // doubles per species row of spack
 constexpr double T_SAFE_LO = 250.0, T_SAFE_HI = 4500.0;  // window in which the fast rows need no exp range checks                 // temperature intervals (distinct t_mid values + 1)
 
 // Device view of the packed mechanism (all pointers into one device arena; passed by value to kernels).
@@ -35,7 +36,8 @@ struct MechDev {
   const double* nlo;          // [7][K] NASA-7, T <= t_mid
   const double* nhi;          // [7][K]
   const double* tmid;         // [K]
-  const double* spack;        // [K][16] AoS for smem staging: W, 1/W, t_mid, 0, lo a1..a6, hi a1..a6
+  const double* spack;        // [K][SPS] AoS for smem staging: W, 1/W, t_mid, 0; cp/R coefficients a1..a5 (low range,
+                              //   high range); H/RT coefficients a1, a2/2, a3/3, a4/4, a5/5, a6 (low, high); 2 pad
   const double* lnA;          // [R]  Eq. 15: ln k_f = lnA + beta lnT - Ta/T
   const double* beta;         // [R]
   const double* Ta;           // [R]  Ea / R_cal

@@ -276,11 +276,16 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
       for (int x = 0; x < ne; ++x) { w |= (uint64_t)espec[e0 + x] << (4 + 10 * x); q[8 + x] = eval1[e0 + x]; }
     std::memcpy(&q[7], &w, sizeof w);
   }
-  std::vector<double> spack((size_t)K * 16, 0.0);
+  std::vector<double> spack((size_t)K * SPS, 0.0);
   for (int k = 0; k < K; ++k) {
-    double* q = &spack[(size_t)k * 16];
+    double* q = &spack[(size_t)k * SPS];
     q[0] = W[k]; q[1] = invW[k]; q[2] = tmid[k];
-    for (int j = 0; j < 6; ++j) { q[4 + j] = d->nasa_lo[7 * k + j]; q[10 + j] = d->nasa_hi[7 * k + j]; }
+    const double hs[5] = {1.0, 0.5, 1.0 / 3.0, 0.25, 0.2};
+    for (int rg = 0; rg < 2; ++rg) {
+      const double* a = rg ? &d->nasa_hi[7 * k] : &d->nasa_lo[7 * k];
+      for (int j = 0; j < 5; ++j) { q[4 + 5 * rg + j] = a[j]; q[14 + 6 * rg + j] = a[j] * hs[j]; }
+      q[14 + 6 * rg + 5] = a[5];
+    }
   }
   std::vector<int> tptr(K + 1, 0), tent;
   for (int k = 0; k < K; ++k) {

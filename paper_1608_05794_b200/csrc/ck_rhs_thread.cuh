@@ -45,13 +45,17 @@ __host__ __device__ inline size_t rhs_smem_bytes(int K, int rstride, int block) 
   return ((size_t)2 * (K + 1) * block + (size_t)rhs_stage_doubles(rstride)) * sizeof(double);
 }
 
-// cp/R and H/(RT) from a staged species row (spack layout: W, 1/W, t_mid, 0, lo a1..a6, hi a1..a6)
-__device__ __forceinline__ void thermo_row(const double* __restrict__ row, const TState& t, double& cpR, double& hRT) {
-  const double* a = row + ((t.T > row[2]) ? 10 : 4);
+// cp/R resp. H/(RT) from a staged species row (spack layout, ck_internal.h): the H/RT coefficients are stored
+// pre-divided (a2/2, a3/3, ...), and each of the two species loops evaluates only the polynomial it needs
+__device__ __forceinline__ double thermo_row_cp(const double* __restrict__ row, const TState& t) {
+  const double* a = row + ((t.T > row[2]) ? 9 : 4);
   const double T = t.T;
-  const double a1 = a[0], a2 = a[1], a3 = a[2], a4 = a[3], a5 = a[4], a6 = a[5];
-  cpR = fma(fma(fma(fma(a5, T, a4), T, a3), T, a2), T, a1);
-  hRT = fma(fma(fma(fma(a5 * 0.2, T, a4 * 0.25), T, a3 * (1.0 / 3.0)), T, a2 * 0.5), T, a1) + a6 * t.invT;
+  return fma(fma(fma(fma(a[4], T, a[3]), T, a[2]), T, a[1]), T, a[0]);
+}
+__device__ __forceinline__ double thermo_row_h(const double* __restrict__ row, const TState& t) {
+  const double* a = row + ((t.T > row[2]) ? 20 : 14);
+  const double T = t.T;
+  return fma(fma(fma(fma(a[4], T, a[3]), T, a[2]), T, a[1]), T, a[0]) + a[5] * t.invT;
 }
 
 // Four reactions with six distinct slot species each, all in flight: rate constants, products, then the
@@ -101,16 +105,14 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
     __syncthreads();
-    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    for (int idx = tid; idx < nk * SPS; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * SPS + idx);
     __syncthreads();
 #pragma unroll 8
     for (int j = 0; j < nk; ++j) {
-      const double* row = stage + j * 16;
+      const double* row = stage + j * SPS;
       const double yw = yin[(size_t)(k0 + j + 1) * ldin] * row[1];
-      double cpR, hRT;
-      thermo_row(row, t, cpR, hRT);
       S += yw;
-      cps = fma(yw, cpR, cps);
+      cps = fma(yw, thermo_row_cp(row, t), cps);
       Cs[(k0 + j) * BLOCK] = yw;
       ws[(k0 + j) * BLOCK] = 0.0;
     }
@@ -176,15 +178,13 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
     __syncthreads();
-    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    for (int idx = tid; idx < nk * SPS; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * SPS + idx);
     __syncthreads();
 #pragma unroll 4
     for (int j = 0; j < nk; ++j) {
-      const double* row = stage + j * 16;
-      double cpR, hRT;
-      thermo_row(row, t, cpR, hRT);
+      const double* row = stage + j * SPS;
       const double w = ws[(k0 + j) * BLOCK];
-      hw = fma(hRT, w, hw);
+      hw = fma(thermo_row_h(row, t), w, hw);
       if (store) fout[(size_t)(k0 + j + 1) * ldout] = w * row[0] * irho;
     }
   }

@@ -103,16 +103,14 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
     __syncthreads();
-    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    for (int idx = tid; idx < nk * SPS; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * SPS + idx);
     __syncthreads();
 #pragma unroll 4
     for (int j = 0; j < nk; ++j) {
-      const double* row = stage + j * 16;
+      const double* row = stage + j * SPS;
       const double yw = yin[(size_t)(k0 + j + 1) * ldin] * row[1];
-      double cpR, hRT;
-      thermo_row(row, t, cpR, hRT);
       S += yw;
-      cps = fma(yw, cpR, cps);
+      cps = fma(yw, thermo_row_cp(row, t), cps);
       Cs[(k0 + j) * BLOCK] = yw;
       tm_st2(wt + 2 * (k0 + j), 0.0);
     }
@@ -172,7 +170,7 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
     __syncthreads();
-    for (int idx = tid; idx < nk * 16; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * 16 + idx);
+    for (int idx = tid; idx < nk * SPS; idx += BLOCK) stage[idx] = __ldg(m.spack + (size_t)k0 * SPS + idx);
     __syncthreads();
     for (int j0 = 0; j0 < nk; j0 += 4) {  // four accumulators per tensor-memory round trip
       uint32_t lo[4], hi[4];
@@ -183,11 +181,9 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
 #pragma unroll
       for (int u = 0; u < 4; ++u)
         if (j0 + u < nk) {
-          const double* row = stage + (j0 + u) * 16;
-          double cpR, hRT;
-          thermo_row(row, t, cpR, hRT);
+          const double* row = stage + (j0 + u) * SPS;
           const double w = __hiloint2double((int)hi[u], (int)lo[u]);
-          hw = fma(hRT, w, hw);
+          hw = fma(thermo_row_h(row, t), w, hw);
           if (store) fout[(size_t)(k0 + j0 + u + 1) * ldout] = w * row[0] * irho;
         }
     }
