@@ -197,7 +197,9 @@ __global__ void __launch_bounds__(BLOCK, 1) rhs_kernel_tmem(const MechDev m, lon
                                                             double* __restrict__ f, long long ldf) {
   extern __shared__ double sm[];
   __shared__ uint32_t s_tmem;
-  const int tid = threadIdx.x, warp = tid >> 5;
+  // warp index broadcast from lane 0: tells the compiler it is warp-uniform, so the tensor-memory addresses below stay
+  // in uniform registers
+  const int tid = threadIdx.x, warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
   if (warp == 0) {  // one warp allocates all 512 columns (one CTA per SM: shared memory is full anyway)
     const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s_tmem);
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst));
