@@ -162,24 +162,32 @@ __device__ __forceinline__ RxnConst load_rxn_global(const MechDev& m, int r, int
 // intervals (the common case) BOTH coefficient sets are read with warp-uniform addresses and selected per lane:
 // lanes of one warp sit in different intervals almost always (independent reactors), and a per-lane address
 // would split every 16-byte broadcast into several shared-memory wavefronts.
+// PRE: slots 0, 1, 3, 4 come back as the pre-shifted words (slot << 12) of the row header, slots 2 and 5 are not decoded
+template <bool PRE = false>
 __device__ __forceinline__ RxnConst load_rxn_row(const double* row, int tint, int nT = 0) {
   RxnConst k;
   const double2 a = *reinterpret_cast<const double2*>(row);
   const double2 b = *reinterpret_cast<const double2*>(row + 2);
   k.lnA = a.x; k.beta = a.y; k.Ta = b.x;
   const unsigned lo = (unsigned)__double2loint(b.y), hi = (unsigned)__double2hiint(b.y);
-  k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
-  k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  if (PRE) {
+    const uint4 w = *reinterpret_cast<const uint4*>(row + 4);
+    k.slot[0] = (int)w.x; k.slot[1] = (int)w.y; k.slot[3] = (int)w.z; k.slot[4] = (int)w.w;
+    k.slot[2] = k.slot[5] = 0;
+  } else {
+    k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
+    k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
+  }
   k.dup = (int)(hi >> 31);
   if (nT == 2) {
-    const double2* c = reinterpret_cast<const double2*>(row + 4);
+    const double2* c = reinterpret_cast<const double2*>(row + RPH);
     const double2 l01 = c[0], l23 = c[1], l45 = c[2], l67 = c[3], h01 = c[4], h23 = c[5], h45 = c[6], h67 = c[7];
     const bool h = tint != 0;
     k.c0 = h ? h01.x : l01.x; k.c1 = h ? h01.y : l01.y; k.c2 = h ? h23.x : l23.x; k.c3 = h ? h23.y : l23.y;
     k.c4 = h ? h45.x : l45.x; k.c5 = h ? h45.y : l45.y; k.c6 = h ? h67.x : l67.x;
     return k;
   }
-  const double2* c = reinterpret_cast<const double2*>(row + 4 + 8 * tint);
+  const double2* c = reinterpret_cast<const double2*>(row + RPH + 8 * tint);
   const double2 c01 = c[0], c23 = c[1], c45 = c[2], c67 = c[3];
   k.c0 = c01.x; k.c1 = c01.y; k.c2 = c23.x; k.c3 = c23.y; k.c4 = c45.x; k.c5 = c45.y; k.c6 = c67.x;
   return k;

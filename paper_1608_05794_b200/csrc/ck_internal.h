@@ -14,6 +14,7 @@ constexpr double R_U = 8.31446261815324e7;  // erg/(mol K)
 constexpr double R_CAL = 1.98720425864083;  // cal/(mol K)
 constexpr double P_0 = 1.01325e6;           // dyn/cm^2 ("one atmosphere")
 constexpr int MAX_TINT = 8;
+constexpr int RPH = 6;   // header doubles of an rpack row
 constexpr int SPS = 28;  // doubles per species row of spack
 constexpr double T_SAFE_LO = 250.0, T_SAFE_HI = 4500.0;  // window in which the fast rows need no exp range checks                 // temperature intervals (distinct t_mid values + 1)
 
@@ -45,8 +46,10 @@ struct MechDev {
   const int* slot;            // [6][R]  slots 0-2 reactants, 3-5 products (species index or K)
   const int* rflag;           // [R]  bit 0: a species sits in two slots of the reaction
   const double* rpack;        // [R][rstride] AoS for smem staging: lnA, beta, Ta, slots (6 x 10 bit in the
-                              //   low/high 32-bit words), then per interval 8 doubles: c0..c6, 0
-  int rstride;                // = 4 + 8 nT
+                              //   low/high 32-bit words), slots 0, 1, 3, 4 once more as 32-bit words holding
+                              //   slot << 12 (byte offset of the C column in a 512-thread CTA; >> 11 is the
+                              //   tensor-memory column), then per interval 8 doubles: c0..c6, 0
+  int rstride;                // = RPH + 8 nT
   int n_cfast;                // leading fast rows whose rpack rows also sit in __constant__ memory (0: none)
   const double* xpack;        // [R - r_tb][16] AoS for smem staging of third-body / falloff rows: lnA0, beta0, Ta0,
                               //   Troe a, 1/T***, 1/T*, T**, packed (n_eff | 6 x 10-bit species), 6 x (alpha-1), 0, 0

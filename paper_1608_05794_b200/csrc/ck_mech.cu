@@ -246,7 +246,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
     }
   }
   if (K > 1022) { set_error("ck_mech_load: more than 1022 species"); return CK_EUNSUPPORTED; }
-  const int rstride = 4 + 8 * nT;
+  const int rstride = RPH + 8 * nT;
   std::vector<double> rpack((size_t)std::max(R, 1) * rstride, 0.0);
   std::vector<int> rflag(std::max(R, 1), 0);
   for (int r = 0; r < R; ++r) {
@@ -260,8 +260,11 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
         if (slot[(size_t)s * R + r] != K && slot[(size_t)s * R + r] == slot[(size_t)s2 * R + r]) dup = true;
     if (dup) { w[1] |= 0x80000000u; rflag[r] = 1; }
     std::memcpy(&q[3], w, sizeof w);
+    const uint32_t pre[4] = {(uint32_t)slot[(size_t)0 * R + r] << 12, (uint32_t)slot[(size_t)1 * R + r] << 12,
+                             (uint32_t)slot[(size_t)3 * R + r] << 12, (uint32_t)slot[(size_t)4 * R + r] << 12};
+    std::memcpy(&q[4], pre, sizeof pre);
     for (int t = 0; t < nT; ++t)
-      for (int j = 0; j < 7; ++j) q[4 + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];
+      for (int j = 0; j < 7; ++j) q[RPH + 8 * t + j] = krc[((size_t)t * 7 + j) * R + r];
   }
   const int n_special = R - r_tb;
   std::vector<double> xpack((size_t)std::max(n_special, 1) * 16, 0.0);

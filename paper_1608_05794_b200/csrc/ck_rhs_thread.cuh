@@ -25,12 +25,12 @@ __device__ __forceinline__ RxnConst load_rxn_cpack(int base, int tint, int nT) {
   k.dup = (int)(hi >> 31);
   if (nT == 2) {
     const bool h = tint != 0;
-    k.c0 = h ? c_pack[base + 12] : c_pack[base + 4]; k.c1 = h ? c_pack[base + 13] : c_pack[base + 5];
-    k.c2 = h ? c_pack[base + 14] : c_pack[base + 6]; k.c3 = h ? c_pack[base + 15] : c_pack[base + 7];
-    k.c4 = h ? c_pack[base + 16] : c_pack[base + 8]; k.c5 = h ? c_pack[base + 17] : c_pack[base + 9];
-    k.c6 = h ? c_pack[base + 18] : c_pack[base + 10];
+    k.c0 = h ? c_pack[base + RPH + 8] : c_pack[base + RPH]; k.c1 = h ? c_pack[base + RPH + 9] : c_pack[base + RPH + 1];
+    k.c2 = h ? c_pack[base + RPH + 10] : c_pack[base + RPH + 2]; k.c3 = h ? c_pack[base + RPH + 11] : c_pack[base + RPH + 3];
+    k.c4 = h ? c_pack[base + RPH + 12] : c_pack[base + RPH + 4]; k.c5 = h ? c_pack[base + RPH + 13] : c_pack[base + RPH + 5];
+    k.c6 = h ? c_pack[base + RPH + 14] : c_pack[base + RPH + 6];
   } else {
-    const int o = base + 4 + 8 * tint;
+    const int o = base + RPH + 8 * tint;
     k.c0 = c_pack[o]; k.c1 = c_pack[o + 1]; k.c2 = c_pack[o + 2]; k.c3 = c_pack[o + 3];
     k.c4 = c_pack[o + 4]; k.c5 = c_pack[o + 5]; k.c6 = c_pack[o + 6];
   }

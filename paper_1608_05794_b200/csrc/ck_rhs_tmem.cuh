@@ -38,16 +38,21 @@ __host__ __device__ inline size_t rhs_tmem_smem_bytes(int K, int rstride, int bl
 template <int BLOCK, int NG, bool B22, bool NC>
 __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const TState& t, int K,
                                                 const double* __restrict__ Cs, uint32_t wt) {
+  static_assert(!B22 || BLOCK == 512, "pre-shifted slot words assume 4096-byte C columns");
   double q[NG];
 #pragma unroll
   for (int u = 0; u < NG; ++u) {
     double kf, kr;
     rate_constants<NC>(kc[u], t, kf, kr);
-    double pf = Cs[kc[u].slot[0] * BLOCK], pr = Cs[kc[u].slot[3] * BLOCK];
-    if (B22) {
-      pf *= Cs[kc[u].slot[1] * BLOCK];
-      pr *= Cs[kc[u].slot[4] * BLOCK];
+    double pf, pr;
+    if (B22) {  // slot words are byte offsets of the C columns
+      const char* Cb = reinterpret_cast<const char*>(Cs);
+      pf = *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[0]) *
+           *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[1]);
+      pr = *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[3]) *
+           *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[4]);
     } else {
+      pf = Cs[kc[u].slot[0] * BLOCK]; pr = Cs[kc[u].slot[3] * BLOCK];
       if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
       if (kc[u].slot[2] != K) pf *= Cs[kc[u].slot[2] * BLOCK];
       if (kc[u].slot[4] != K) pr *= Cs[kc[u].slot[4] * BLOCK];
@@ -60,13 +65,14 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
     uint32_t lo[6], hi[6];
 #pragma unroll
     for (int s = 0; s < 6; ++s)
-      if (B22 ? (s != 2 && s != 5) : (s == 0 || s == 3 || kc[u].slot[s] != K)) tm_ld2_raw(wt + 2 * kc[u].slot[s], lo[s], hi[s]);
+      if (B22 ? (s != 2 && s != 5) : (s == 0 || s == 3 || kc[u].slot[s] != K))
+        tm_ld2_raw(wt + (B22 ? (unsigned)kc[u].slot[s] >> 11 : 2u * kc[u].slot[s]), lo[s], hi[s]);
     tm_wait_ld();
 #pragma unroll
     for (int s = 0; s < 6; ++s)
       if (B22 ? (s != 2 && s != 5) : (s == 0 || s == 3 || kc[u].slot[s] != K)) {
         const double w = __hiloint2double((int)hi[s], (int)lo[s]);
-        tm_st2(wt + 2 * kc[u].slot[s], (s < 3) ? w - q[u] : w + q[u]);
+        tm_st2(wt + (B22 ? (unsigned)kc[u].slot[s] >> 11 : 2u * kc[u].slot[s]), (s < 3) ? w - q[u] : w + q[u]);
       }
     tm_wait_st();
   }
@@ -79,7 +85,7 @@ __device__ __forceinline__ void fast_rows_tmem(const double* __restrict__ stage,
   for (int j = 0; j < n22; j += 4) {
     RxnConst kc[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row(stage + (j + u) * rs, t.tint);
+    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row<true>(stage + (j + u) * rs, t.tint);
     fast_group_tmem<BLOCK, 4, true, NC>(kc, t, K, Cs, wt);
   }
   for (int j = n22; j < nfast; j += 2) {

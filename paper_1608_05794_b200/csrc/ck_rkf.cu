@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;");
-    const int warp = tid >> 5;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // warp-uniform for the compiler (ck_rhs_tmem.cuh)
     wt = s_tmem + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * (m.K + 1));
   }
   const long long slot = (long long)blockIdx.x * BLOCK + tid;
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
     lane_act += act; lane_tot += 1;
     // ---- one RHS evaluation for every lane: f(stage argument) -> evaluation vector of this stage -----
     const int dstv = (st < 0) ? (st + 3) : (st + 1);  // H0A -> 1, H0B -> 2, stage s -> s+1
-    if (TM) rhs_thread_tmem<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wt, stage_buf, act);
+    if constexpr (TM) rhs_thread_tmem<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wt, stage_buf, act);
     else rhs_thread<BLOCK>(m, Vy + 7 * vs, ns, p, Vy + (size_t)dstv * vs, ns, Cs, wsm, stage_buf, act);
     if (!act) continue;
     c_rhs++;
