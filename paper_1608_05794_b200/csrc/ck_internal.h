@@ -27,7 +27,8 @@ constexpr double T_SAFE_LO = 250.0, T_SAFE_HI = 4500.0;  // window in which the 
 // accumulator at K), so rate products and the omega scatter are branch-free.
 struct MechDev {
   int K, R, nT;
-  int r_22;                   // leading rows of the plain group that are A + B <=> C + D with four distinct species
+  int r_22;                   // leading rows of the plain group with at most two reactants and two products, all
+                              //   distinct (A + B <=> C + D; a missing partner is the dummy species K)
   int r_dup, r_tb, r_lind, r_troe;
   int r_tbf;                  // [r_tb, r_tbf): three-body rows with distinct slot species, bounded exponents, <= 6 efficiencies
   double t_safe_lo, t_safe_hi;  // see ck_mech.cu `bounded`

@@ -88,11 +88,16 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   auto has_dup = [&](int i) {
     for (int x = d->reac_ptr[i]; x < d->reac_ptr[i + 1]; ++x) {
       if (d->reac_nu[x] != 1) return true;
+      for (int x2 = d->reac_ptr[i]; x2 < x; ++x2)
+        if (d->reac_spec[x2] == d->reac_spec[x]) return true;
       for (int y = d->prod_ptr[i]; y < d->prod_ptr[i + 1]; ++y)
         if (d->prod_spec[y] == d->reac_spec[x]) return true;
     }
-    for (int y = d->prod_ptr[i]; y < d->prod_ptr[i + 1]; ++y)
+    for (int y = d->prod_ptr[i]; y < d->prod_ptr[i + 1]; ++y) {
       if (d->prod_nu[y] != 1) return true;
+      for (int y2 = d->prod_ptr[i]; y2 < y; ++y2)
+        if (d->prod_spec[y2] == d->prod_spec[y]) return true;
+    }
     return false;
   };
   std::vector<int> perm;
@@ -136,7 +141,9 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   };
   std::vector<char> slow(R, 0);
   for (int i = 0; i < R; ++i) slow[i] = (d->type[i] != 0) || has_dup(i) || !bounded(i);
-  auto is22 = [&](int i) { return d->reac_ptr[i + 1] - d->reac_ptr[i] == 2 && d->prod_ptr[i + 1] - d->prod_ptr[i] == 2; };
+  // at most two reactants and two products (all distinct, nu = 1): slots 0, 1, 3, 4 only; a missing partner is the
+  // dummy species K (C[K] = 1, accumulator column K is a sink), so the group runs without predicates
+  auto is22 = [&](int i) { return d->reac_ptr[i + 1] - d->reac_ptr[i] <= 2 && d->prod_ptr[i + 1] - d->prod_ptr[i] <= 2; };
   int r_22 = 0;
   for (int i = 0; i < R; ++i) if (!slow[i] && is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; r_22++; }
   for (int i = 0; i < R; ++i) if (!slow[i] && !is22(i)) { perm.push_back(i); cnt[0]++; r_dup++; }
