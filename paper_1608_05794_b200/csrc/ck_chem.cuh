@@ -213,7 +213,9 @@ struct RateAux {
 };
 
 // Rate of progress q_i of regrouped reaction r.  WANT_AUX also fills the derivative pieces.
-template <int CS, bool WANT_AUX>
+// TYPE >= 0 fixes the row kind at compile time (0 plain, 1 three-body, 2 Lindemann, 3 Troe) and promises a staged
+// xrow; TYPE < 0 reads the kind off the group boundaries.
+template <int CS, bool WANT_AUX, int TYPE = -1>
 __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnConst& k, const TState& t,
                                              const double* __restrict__ C, double Ctot, RateAux* aux,
                                              const double* __restrict__ xrow = nullptr) {
@@ -224,11 +226,11 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
   double kf, kr;
   rate_constants(k, t, kf, kr);
   double ci = 1.0, dci_dM = 0.0, dci_dT = 0.0;
-  if (r >= m.r_tb) {  // third-body / falloff factor c_i (reading G9)
+  if (TYPE < 0 ? (r >= m.r_tb) : (TYPE >= 1)) {  // third-body / falloff factor c_i (reading G9)
     const int j = r - m.r_tb;
     double M = Ctot;
     // constants of this row: from the staged xpack row (shared memory) when given, else from global memory
-    const double* xr = xrow ? xrow : m.xpack + (size_t)j * 16;
+    const double* xr = (TYPE >= 0 || xrow) ? xrow : m.xpack + (size_t)j * 16;
     const unsigned long long xw = (unsigned long long)__double_as_longlong(xr[7]);
     const int ne = (int)(xw & 15ull);
     if (ne != 15) {
@@ -237,7 +239,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
       for (int e = __ldg(m.eptr + j), e1 = __ldg(m.eptr + j + 1); e < e1; ++e)
         M = fma(__ldg(m.eval1 + e), C[(size_t)__ldg(m.espec + e) * CS], M);
     }
-    if (r < m.r_lind) {
+    if (TYPE < 0 ? (r < m.r_lind) : (TYPE == 1)) {
       ci = M;
       if (WANT_AUX) dci_dM = 1.0;
     } else {
@@ -248,7 +250,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
       const double inv1p = ck_rcp(1.0 + Pr);
       const double L = Pr * inv1p;  // Lindemann
       double F = 1.0, dlnF_dlP = 0.0, dlnF_dT = 0.0;
-      if (r >= m.r_troe) {
+      if (TYPE < 0 ? (r >= m.r_troe) : (TYPE == 3)) {
         const double a = xr[3], i3 = xr[4], i1 = xr[5], T2 = xr[6];
         const double e3 = ck_exp(-T * i3), e1 = ck_exp(-T * i1);
         double Fc = fma(1.0 - a, e3, a * e1);

@@ -96,6 +96,39 @@ __device__ __forceinline__ void fast_rows_tmem(const double* __restrict__ stage,
   }
 }
 
+// one row outside the fast groups (kind TYPE, reaction_q): rate of progress, then the omega scatter
+template <int BLOCK, int TYPE>
+__device__ __forceinline__ void slow_row_tmem(const MechDev& m, int r, const double* __restrict__ row,
+                                              const double* __restrict__ xrow, const TState& t,
+                                              const double* __restrict__ Cs, double Ctot, uint32_t wt) {
+  const int K = m.K;
+  const RxnConst kc = load_rxn_row(row, t.tint);
+  const double q = reaction_q<BLOCK, false, TYPE>(m, r, kc, t, Cs, Ctot, nullptr, xrow);
+  if (!kc.dup) {  // six distinct slot species: one tensor-memory round trip
+    uint32_t lo[6], hi[6];
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc.slot[s] != K) tm_ld2_raw(wt + 2 * kc.slot[s], lo[s], hi[s]);
+    tm_wait_ld();
+#pragma unroll
+    for (int s = 0; s < 6; ++s)
+      if (s == 0 || s == 3 || kc.slot[s] != K) {
+        const double w = __hiloint2double((int)hi[s], (int)lo[s]);
+        tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+      }
+    tm_wait_st();
+  } else {
+#pragma unroll
+    for (int s = 0; s < 6; ++s) {  // slot by slot: a species sits in two slots
+      double w;
+      tm_ld2(wt + 2 * kc.slot[s], w);
+      tm_wait_ld();
+      tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
+      tm_wait_st();
+    }
+  }
+}
+
 template <int BLOCK>
 __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
                                                 double* __restrict__ fout, long long ldout, double* __restrict__ Cs,
@@ -142,34 +175,13 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     const int nfast = n22 + (max(0, min(nr, m.r_dup - r0) - n22) & ~1);
     if (allsafe) fast_rows_tmem<BLOCK, true>(stage, rs, n22, nfast, t, K, Cs, wt);
     else fast_rows_tmem<BLOCK, false>(stage, rs, n22, nfast, t, K, Cs, wt);
-    for (int j = nfast; j < nr; ++j) {
-      const RxnConst kc = load_rxn_row(stage + j * rs, t.tint);
-      const int r = r0 + j;
-      const double q = reaction_q<BLOCK, false>(m, r, kc, t, Cs, Ctot, nullptr, xstage + (r >= x0 ? (r - x0) * 16 : 0));
-      if (!kc.dup) {  // six distinct slot species: one tensor-memory round trip
-        uint32_t lo[6], hi[6];
-#pragma unroll
-        for (int s = 0; s < 6; ++s)
-          if (s == 0 || s == 3 || kc.slot[s] != K) tm_ld2_raw(wt + 2 * kc.slot[s], lo[s], hi[s]);
-        tm_wait_ld();
-#pragma unroll
-        for (int s = 0; s < 6; ++s)
-          if (s == 0 || s == 3 || kc.slot[s] != K) {
-            const double w = __hiloint2double((int)hi[s], (int)lo[s]);
-            tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
-          }
-        tm_wait_st();
-      } else {
-#pragma unroll
-        for (int s = 0; s < 6; ++s) {  // slot by slot: a species sits in two slots
-          double w;
-          tm_ld2(wt + 2 * kc.slot[s], w);
-          tm_wait_ld();
-          tm_st2(wt + 2 * kc.slot[s], (s < 3) ? w - q : w + q);
-          tm_wait_st();
-        }
-      }
-    }
+    // the rest of the chunk one row at a time, one loop per row kind (the groups are contiguous)
+    const int j1 = min(nr, max(nfast, m.r_tb - r0)), j2 = min(nr, max(nfast, m.r_lind - r0)),
+              j3 = min(nr, max(nfast, m.r_troe - r0));
+    for (int j = nfast; j < j1; ++j) slow_row_tmem<BLOCK, 0>(m, r0 + j, stage + j * rs, nullptr, t, Cs, Ctot, wt);
+    for (int j = j1; j < j2; ++j) slow_row_tmem<BLOCK, 1>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
+    for (int j = j2; j < j3; ++j) slow_row_tmem<BLOCK, 2>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
+    for (int j = j3; j < nr; ++j) slow_row_tmem<BLOCK, 3>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
   }
   const double irho = 1.0 / rho;
   double hw = 0.0;
