@@ -96,14 +96,8 @@ __device__ __forceinline__ void fast_rows_tmem(const double* __restrict__ stage,
   }
 }
 
-// one row outside the fast groups (kind TYPE, reaction_q): rate of progress, then the omega scatter
-template <int BLOCK, int TYPE>
-__device__ __forceinline__ void slow_row_tmem(const MechDev& m, int r, const double* __restrict__ row,
-                                              const double* __restrict__ xrow, const TState& t,
-                                              const double* __restrict__ Cs, double Ctot, uint32_t wt) {
-  const int K = m.K;
-  const RxnConst kc = load_rxn_row(row, t.tint);
-  const double q = reaction_q<BLOCK, false, TYPE>(m, r, kc, t, Cs, Ctot, nullptr, xrow);
+// omega scatter of one row outside the fast groups
+__device__ __forceinline__ void slow_scatter_tmem(const RxnConst& kc, double q, int K, uint32_t wt) {
   if (!kc.dup) {  // six distinct slot species: one tensor-memory round trip
     uint32_t lo[6], hi[6];
 #pragma unroll
@@ -127,6 +121,23 @@ __device__ __forceinline__ void slow_row_tmem(const MechDev& m, int r, const dou
       tm_wait_st();
     }
   }
+}
+
+// NP consecutive rows of kind TYPE outside the fast groups (reaction_q): rates of progress first (independent chains
+// the scheduler can interleave), then the scatters in row order
+template <int BLOCK, int TYPE, int NP>
+__device__ __forceinline__ void slow_rows_tmem(const MechDev& m, int r, const double* __restrict__ row, int rs,
+                                               const double* __restrict__ xrow, const TState& t,
+                                               const double* __restrict__ Cs, double Ctot, uint32_t wt) {
+  RxnConst kc[NP];
+  double q[NP];
+#pragma unroll
+  for (int u = 0; u < NP; ++u) {
+    kc[u] = load_rxn_row(row + u * rs, t.tint);
+    q[u] = reaction_q<BLOCK, false, TYPE>(m, r + u, kc[u], t, Cs, Ctot, nullptr, xrow + u * 16);
+  }
+#pragma unroll
+  for (int u = 0; u < NP; ++u) slow_scatter_tmem(kc[u], q[u], m.K, wt);
 }
 
 template <int BLOCK>
@@ -178,10 +189,13 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     // the rest of the chunk one row at a time, one loop per row kind (the groups are contiguous)
     const int j1 = min(nr, max(nfast, m.r_tb - r0)), j2 = min(nr, max(nfast, m.r_lind - r0)),
               j3 = min(nr, max(nfast, m.r_troe - r0));
-    for (int j = nfast; j < j1; ++j) slow_row_tmem<BLOCK, 0>(m, r0 + j, stage + j * rs, nullptr, t, Cs, Ctot, wt);
-    for (int j = j1; j < j2; ++j) slow_row_tmem<BLOCK, 1>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
-    for (int j = j2; j < j3; ++j) slow_row_tmem<BLOCK, 2>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
-    for (int j = j3; j < nr; ++j) slow_row_tmem<BLOCK, 3>(m, r0 + j, stage + j * rs, xstage + (r0 + j - x0) * 16, t, Cs, Ctot, wt);
+    const double* xs = xstage - (size_t)(x0 - r0) * 16;  // xs + 16 j: falloff row of chunk row j
+    int j = nfast;
+    for (; j < j1; ++j) slow_rows_tmem<BLOCK, 0, 1>(m, r0 + j, stage + j * rs, rs, xs, t, Cs, Ctot, wt);
+    for (; j + 1 < j2; j += 2) slow_rows_tmem<BLOCK, 1, 2>(m, r0 + j, stage + j * rs, rs, xs + 16 * j, t, Cs, Ctot, wt);
+    for (; j < j2; ++j) slow_rows_tmem<BLOCK, 1, 1>(m, r0 + j, stage + j * rs, rs, xs + 16 * j, t, Cs, Ctot, wt);
+    for (; j < j3; ++j) slow_rows_tmem<BLOCK, 2, 1>(m, r0 + j, stage + j * rs, rs, xs + 16 * j, t, Cs, Ctot, wt);
+    for (; j < nr; ++j) slow_rows_tmem<BLOCK, 3, 1>(m, r0 + j, stage + j * rs, rs, xs + 16 * j, t, Cs, Ctot, wt);
   }
   const double irho = 1.0 / rho;
   double hw = 0.0;
