@@ -21,12 +21,32 @@ def _deps():
         [os.path.join(_HERE, "..", "include", "ck.h")]
 
 
+def _compile_one(nvcc, src, obj, verbose):
+    cmd = [nvcc] + [f for f in NVCC_FLAGS if f != "-shared"] + (["-Xptxas", "-v"] if verbose else []) + \
+        ["-c", "-o", obj, src]
+    subprocess.run(cmd, check=True, cwd=CSRC)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in _deps()):
+    """One object per .cu (compiled in parallel, reused while newer than every header), then one link."""
+    deps = _deps()
+    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(s) for s in deps):
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + sources() + ["-lcudart"]
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    objdir = os.path.join(_HERE, "build")
+    os.makedirs(objdir, exist_ok=True)
+    hdr_time = max(os.path.getmtime(s) for s in deps if not s.endswith(".cu"))
+    jobs, objs = [], []
+    for src in sources():
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        objs.append(obj)
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
+            jobs.append((src, obj))
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as ex:
+        for f in [ex.submit(_compile_one, nvcc, s, o, verbose) for s, o in jobs]:
+            f.result()
+    subprocess.run([nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"], check=True, cwd=CSRC)
     return LIB
 
 
