@@ -30,7 +30,7 @@ UNIT = "RHS evals/s"
 # FP64 vector peak derived from unit counts and clocks:
 # 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
 PEAK_SLOTS = 148 * 64 * 1.965e9
-RHS_DRAM_BYTES_PER_STATE = 683.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
+RHS_DRAM_BYTES_PER_STATE = 690.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
 
 
 class ClockSampler:
