@@ -46,7 +46,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as ex:
         for f in [ex.submit(_compile_one, nvcc, s, o, verbose) for s, o in jobs]:
             f.result()
-    subprocess.run([nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"], check=True, cwd=CSRC)
+    subprocess.run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs + ["-lcudart"], check=True, cwd=CSRC)
     return LIB
 
 

@@ -319,6 +319,102 @@ __device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int 
   return ok;
 }
 
+// Segmented register-resident factorisation for compile-time N <= G: thread tid < N holds row tid of the matrix in
+// registers (as lu_factor_rows), but the step loop is a RUNTIME loop inside compile-time column segments of length S,
+// so the code is N/S loop bodies instead of N unrolled steps (the fully unrolled variant is instruction-fetch
+// bound).  Inside segment [J0, J0+S) every step updates ALL columns j >= J0 of the register row: columns <= k are
+// dead registers by then (their multipliers were stored to shared memory when they were computed), so whatever the
+// update leaves there is never read.  The rank-1 update therefore costs one broadcast shared-memory load per FMA
+// instead of two loads and a store, which is what bounded lu_factor_rows_smem (shared-memory pipe).
+// Publishing the pivot row: after the warp stage of the pivot search, each warp's own best candidate row copies its
+// live registers (columns >= k) to its shared-memory row BEFORE the cross-warp exchange, so one barrier per step
+// serves both the exchange and the row; a warp candidate that loses has only refreshed dead storage.
+// Layout on return is that of lu_factor_rows_smem: A[i][k] = multiplier for k < pstep_i, U beyond, dinv[k] = 1/U_kk.
+// x if i == j else y, opaque to the optimiser: written as a C++ conditional over the columns of the register row,
+// nvcc recognises the chain as a dynamically indexed array read and moves the whole row to local memory.
+__device__ __forceinline__ double sel_eq_f64(int i, int j, double x, double y) {
+  double r;
+  asm("{\n\t.reg .pred p;\n\tsetp.eq.s32 p, %1, %2;\n\tselp.f64 %0, %3, %4, p;\n\t}" : "=d"(r) : "r"(i), "r"(j), "d"(x), "d"(y));
+  return r;
+}
+
+template <int N, int G, int S, int J0>
+__device__ __forceinline__ void lu_factor_seg(double (&a)[N], int& pstep, double& cand, double& cinv, double* __restrict__ A,
+                                              int lda, double* __restrict__ dinv, double* red2, bool& ok) {
+  if constexpr (J0 < N) {
+    constexpr int J1 = (J0 + S < N) ? J0 + S : N;
+    constexpr int W = G / 32;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    double* row = A + (size_t)(tid < N ? tid : 0) * lda;
+#pragma unroll 1
+    for (int k = J0; k < J1; ++k) {
+      const double v = (pstep == -1) ? fabs(cand) : -1.0;
+      const unsigned hi = (v >= 0.0 || v != v) ? (unsigned)__double2hiint(fabs(v)) + 1u : 0u;
+      const unsigned lo = (unsigned)__double2loint(v);
+      const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
+      const unsigned lo2 = (hi == mh) ? lo : 0u;
+      const unsigned ml = __reduce_max_sync(0xffffffffu, lo2);
+      const unsigned win = __ballot_sync(0xffffffffu, hi == mh && lo2 == ml);
+      const int wl = __ffs(win) - 1;
+      if (lane == wl && pstep == -1) {
+#pragma unroll
+        for (int j = J0; j < N; ++j)
+          if (j >= J1 || j >= k) row[j] = a[j];
+      }
+      int p = (w << 5) + wl;
+      double ipv = __shfl_sync(0xffffffffu, cinv, wl);
+      if constexpr (W == 1) {
+        __syncwarp();
+      } else {
+        double* base = red2 + (k & 1) * 4 * W;
+        unsigned* rk = reinterpret_cast<unsigned*>(base);  // [W][2] keys
+        int* ri = reinterpret_cast<int*>(base + W);        // [W] rows
+        double* rinv = base + 2 * W;                       // [W] reciprocals
+        if (lane == 0) { rk[2 * w] = mh; rk[2 * w + 1] = ml; ri[w] = p; rinv[w] = ipv; }
+        __syncthreads();
+        unsigned bh = rk[0], bl = rk[1];
+        p = ri[0]; ipv = rinv[0];
+#pragma unroll
+        for (int i = 1; i < W; ++i) {
+          const unsigned h2 = rk[2 * i], l2 = rk[2 * i + 1];
+          if (h2 > bh || (h2 == bh && l2 > bl)) { bh = h2; bl = l2; p = ri[i]; ipv = rinv[i]; }
+        }
+      }
+      if (!isfinite(ipv) || ipv == 0.0) ok = false;  // zero / non-finite pivot (uniform)
+      const double* prow = A + (size_t)p * lda;
+      // straight-line update (two warps per CTA: a taken branch costs more than the work it skips).  Rows that are
+      // out (pivot rows, tid >= N) run the FMAs on dead registers; only the stores are predicated.
+      const bool upd = (pstep == -1) && (tid != p);
+      if (tid == p) dinv[k] = ipv;
+      pstep = (tid == p) ? k : pstep;
+      const double l = cand * ipv;
+      if (upd) row[k] = l;
+#pragma unroll
+      for (int j = J0; j < N; ++j) a[j] = fma(-l, prow[j], a[j]);
+      if constexpr (J0 + 1 < N) {  // next step's candidate: column k+1, somewhere in (J0, J1]
+        double c = a[J0 + 1];
+#pragma unroll
+        for (int j = J0 + 2; j <= J1 && j < N; ++j) c = sel_eq_f64(k + 1, j, a[j], c);
+        cand = upd ? c : 1.0;  // rows that are out keep a harmless candidate (no slow path in the reciprocal)
+        cinv = 1.0 / cand;
+      }
+    }
+    lu_factor_seg<N, G, S, J1>(a, pstep, cand, cinv, A, lda, dinv, red2, ok);
+  }
+}
+
+// a: this thread's row (thread tid < N owns row tid; zeros for tid >= N).  red2: 2 x 4 x (G/32) doubles.
+template <int N, int G, int S>
+__device__ __forceinline__ bool lu_factor_rows_seg(double (&a)[N], int& pstep, double* __restrict__ A, int lda,
+                                                   double* __restrict__ dinv, double* red2) {
+  pstep = (threadIdx.x < N) ? -1 : -2;
+  bool ok = true;
+  double cand = a[0], cinv = 1.0 / a[0];
+  lu_factor_seg<N, G, S, 0>(a, pstep, cand, cinv, A, lda, dinv, red2, ok);
+  __syncthreads();
+  return ok;
+}
+
 // b: entry `tid` of the right-hand side on entry, x[pstep] on return.  bs: 2 doubles of shared scratch.
 template <int G>
 __device__ __forceinline__ void lu_solve_rows_smem(const double* __restrict__ A, int lda, int N, int pstep,
@@ -352,6 +448,106 @@ __device__ __forceinline__ void lu_solve_rows_smem(const double* __restrict__ A,
       }
     }
   }
+  __syncthreads();
+}
+
+}  // namespace ck
+
+// ---------------------------------------------------------------------------------------------------------
+// Stage solves, four elimination steps per barrier.  lu_solve_rows_smem spends one barrier round trip per step
+// (2N per solve, ~100 cycles each, nothing to overlap it with); here the owners of four consecutive steps publish
+// their entries of b together, and every thread solves the 4 x 4 triangular diagonal block redundantly from a
+// compact copy of it (Lb / Ub, filled once per factorisation by lu_compact4) before updating its own entry with four
+// FMAs.  The operation order per entry is that of the step-by-step solve, so the results are bit-identical.
+namespace ck {
+
+// Lb[3k + x] = L[p_k][k0 + x] for k0 + x < k,  Ub[3k + x] = U[p_k][k + 1 + x] for k + 1 + x <= k0 + 3  (k0 = k & ~3,
+// p_k the row chosen at step k); zero elsewhere.  Lb, Ub: 3N doubles each.
+template <int G>
+__device__ __forceinline__ void lu_compact4(const double* __restrict__ A, int lda, int N, int pstep, double* __restrict__ Lb,
+                                            double* __restrict__ Ub) {
+  if (pstep >= 0) {
+    const int k = pstep, k0 = k & ~3;
+    const double* row = A + (size_t)threadIdx.x * lda;
+#pragma unroll
+    for (int x = 0; x < 3; ++x) {
+      Lb[3 * k + x] = (k0 + x < k) ? row[k0 + x] : 0.0;
+      const int j = k + 1 + x;
+      Ub[3 * k + x] = (j <= k0 + 3 && j < N) ? row[j] : 0.0;
+    }
+  }
+  __syncthreads();
+}
+
+// One block of NB <= 4 steps of the forward (FWD) or backward substitution; straight-line code (selects, no
+// branches: with two warps per CTA a taken branch costs more than the arithmetic it skips).
+template <int NB, bool FWD>
+__device__ __forceinline__ void lu_solve_block4(const double* __restrict__ row, int k0, int pstep, const double* __restrict__ dinv,
+                                                const double* __restrict__ Lb, const double* __restrict__ Ub, double& b,
+                                                double* __restrict__ bsp) {
+  double l[NB];
+#pragma unroll
+  for (int x = 0; x < NB; ++x) l[x] = row[k0 + x];
+  const int o = pstep - k0;
+  if (o >= 0 && o < NB) bsp[o] = b;
+  __syncthreads();
+  double v[4] = {0.0, 0.0, 0.0, 0.0};
+  if constexpr (FWD) {
+    const double* L = Lb + 3 * k0;
+    v[0] = bsp[0];
+    if constexpr (NB > 1) v[1] = fma(-L[3], v[0], bsp[1]);
+    if constexpr (NB > 2) v[2] = fma(-L[7], v[1], fma(-L[6], v[0], bsp[2]));
+    if constexpr (NB > 3) v[3] = fma(-L[11], v[2], fma(-L[10], v[1], fma(-L[9], v[0], bsp[3])));
+    double upd = b;
+#pragma unroll
+    for (int x = 0; x < NB; ++x) upd = fma(-l[x], v[x], upd);
+    b = (o >= NB) ? upd : b;
+  } else {
+    const double* U = Ub + 3 * k0;
+    if constexpr (NB > 3) v[3] = bsp[3] * dinv[k0 + 3];
+    if constexpr (NB > 2) v[2] = (NB > 3 ? fma(-U[6], v[3], bsp[2]) : bsp[2]) * dinv[k0 + 2];
+    if constexpr (NB > 1) {
+      double t = bsp[1];
+      if constexpr (NB > 3) t = fma(-U[4], v[3], t);
+      if constexpr (NB > 2) t = fma(-U[3], v[2], t);
+      v[1] = t * dinv[k0 + 1];
+    }
+    {
+      double t = bsp[0];
+      if constexpr (NB > 3) t = fma(-U[2], v[3], t);
+      if constexpr (NB > 2) t = fma(-U[1], v[2], t);
+      if constexpr (NB > 1) t = fma(-U[0], v[1], t);
+      v[0] = t * dinv[k0];
+    }
+    double upd = b;
+#pragma unroll
+    for (int x = NB - 1; x >= 0; --x) upd = fma(-l[x], v[x], upd);
+    b = (pstep >= 0 && o < 0) ? upd : b;
+  }
+  b = (o == 0) ? v[0] : b;
+  b = (o == 1) ? v[1] : b;
+  b = (o == 2) ? v[2] : b;
+  b = (o == 3) ? v[3] : b;
+}
+
+// b: entry `tid` of the right-hand side on entry, x[pstep] on return.  bs: 8 doubles of shared scratch.
+template <int G>
+__device__ __forceinline__ void lu_solve_rows_blk(const double* __restrict__ A, int lda, int N, int pstep,
+                                                  const double* __restrict__ dinv, const double* __restrict__ Lb,
+                                                  const double* __restrict__ Ub, double& b, double* __restrict__ bs) {
+  const double* row = A + (size_t)(threadIdx.x < N ? threadIdx.x : 0) * lda;
+  const int Nf = N & ~3, tail = N & 3;
+  int par = 0;
+#pragma unroll 2
+  for (int k0 = 0; k0 < Nf; k0 += 4, par ^= 4) lu_solve_block4<4, true>(row, k0, pstep, dinv, Lb, Ub, b, bs + par);
+  if (tail) {  // the ragged last block, forward then backward (uniform branch, once per solve)
+    if (tail == 1) { lu_solve_block4<1, true>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); par ^= 4; lu_solve_block4<1, false>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); }
+    else if (tail == 2) { lu_solve_block4<2, true>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); par ^= 4; lu_solve_block4<2, false>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); }
+    else { lu_solve_block4<3, true>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); par ^= 4; lu_solve_block4<3, false>(row, Nf, pstep, dinv, Lb, Ub, b, bs + par); }
+    par ^= 4;
+  }
+#pragma unroll 2
+  for (int k0 = Nf - 4; k0 >= 0; k0 -= 4, par ^= 4) lu_solve_block4<4, false>(row, k0, pstep, dinv, Lb, Ub, b, bs + par);
   __syncthreads();
 }
 

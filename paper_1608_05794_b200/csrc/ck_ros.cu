@@ -62,6 +62,19 @@ __device__ __forceinline__ double wrms_coop(const double* v, const double* y, in
   return sqrt(block_sum<G>(s, red) / N);
 }
 
+// ONE out-of-line copy of the plain evaluation f(y) -> f for the integrator's six call sites (EstimateH0 x 2, two
+// stages, FD Jacobian x 2).  Inlined six times it made ros4_kernel ~24 k instructions, and with five CTAs per SM in
+// different phases the kernel ran out of instruction cache (every phase slowed down when any phase's code grew).
+// Arguments are offsets into the CTA's dynamic shared memory so that the callee still sees shared-memory pointers
+// (LDS/STS, not generic accesses); the mechanism is read through the kernel's __grid_constant__ parameter.
+template <int G>
+__device__ __noinline__ void rhs_stage(const MechDev* __restrict__ mp, int y_off, double p, int f_off) {
+  extern __shared__ double sm[];
+  const RosShared s = ros_carve(sm, mp->K, mp->R, G);
+  TState t;
+  rhs_coop<G, false>(*mp, sm + y_off, p, sm + f_off, s.c, t);
+}
+
 // Jacobian of the reactor in s.y into s.A: analytic, or CVODE-style forward differences (PAPER.md:281,
 // reading G12): sigma_j = max(sqrt(eps)|y_j|, sigma_0 (rtol|y_j| + atol)), sigma_0 = 1000 N eps |h| ||f||_wrms.
 // Leaves f(y) in s.f0.  Returns the number of RHS evaluations spent.
@@ -83,7 +96,7 @@ __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, dou
     return 1;
   }
   if (clk_mid) *clk_mid = clock64();
-  rhs_coop<G, false>(m, s.y, p, s.f0, s.c, t);
+  rhs_stage<G>(&m, (int)(s.y - s.A), p, (int)(s.f0 - s.A));
   const double eps = 2.220446049250313e-16;
   const double fn = wrms_coop<G>(s.f0, s.y, N, rtol, atol, s.c.red);
   const double s0 = (fn != 0.0) ? 1000.0 * N * eps * fabs(h) * fn : 1.0;
@@ -95,7 +108,7 @@ __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, dou
     __syncthreads();
     if (tid == 0) s.yt[j] = yj + sig;
     __syncthreads();
-    rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+    rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
     for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + j] = (s.ft[i] - s.f0[i]) / sig;
     if (tid == 0) s.yt[j] = yj;
   }
@@ -104,7 +117,7 @@ __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, dou
 }
 
 template <int G>
-__global__ void __launch_bounds__(G) jac_kernel(const MechDev m, long long n, const double* __restrict__ y, long long ld,
+__global__ void __launch_bounds__(G) jac_kernel(const __grid_constant__ MechDev m, long long n, const double* __restrict__ y, long long ld,
                                                 const double* __restrict__ p, int mode, double h, double rtol, double atol,
                                                 double* __restrict__ J, long long ldJ) {
   extern __shared__ double sm[];
@@ -140,14 +153,14 @@ __device__ __forceinline__ double estimate_h0_coop(const MechDev& m, RosShared& 
                                                    double atol) {
   const int N = m.K + 1, tid = threadIdx.x;
   TState t;
-  rhs_coop<G, false>(m, s.y, p, s.f0, s.c, t);
+  rhs_stage<G>(&m, (int)(s.y - s.A), p, (int)(s.f0 - s.A));
   const double d0 = wrms_coop<G>(s.y, s.y, N, rtol, atol, s.c.red);
   const double d1 = wrms_coop<G>(s.f0, s.y, N, rtol, atol, s.c.red);
   const double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 * dt : 0.01 * d0 / d1;
   __syncthreads();
   for (int i = tid; i < N; i += G) s.yt[i] = fma(ha, s.f0[i], s.y[i]);
   __syncthreads();
-  rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+  rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
   for (int i = tid; i < N; i += G) s.tmp[i] = s.ft[i] - s.f0[i];
   __syncthreads();
   const double d2 = wrms_coop<G>(s.tmp, s.y, N, rtol, atol, s.c.red) / ha;
@@ -180,7 +193,7 @@ __device__ __forceinline__ void solve_rows_smem(const double* __restrict__ A, in
 constexpr int ros_min_ctas(int G) { return G == 32 ? 12 : (G == 64 ? 5 : 1); }
 
 template <int G, int NR, int NS>
-__global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const MechDev m, const RosArgs a) {
+__global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_constant__ MechDev m, const RosArgs a) {
   using namespace ros4c;
   extern __shared__ double sm[];
   __shared__ long long s_next;
@@ -219,13 +232,27 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const MechDev 
       long long k1 = clock64();
       ck[0] += kmid - k0; ck[1] += k1 - kmid;
       const double ihg = 1.0 / (h * gam), ih = 1.0 / h;
-      for (int idx = tid; idx < N * lda; idx += G) s.A[idx] = -s.A[idx];
-      __syncthreads();
-      for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + i] += ihg;
-      __syncthreads();
+      constexpr bool REG_SEG = NS >= 32;             // compile-time N, rows in registers, segmented step loop
+      constexpr bool REG_FULL = NS > 0 && NS < 32;   // compile-time N, rows in registers, fully unrolled
+      if constexpr (!REG_SEG) {
+        for (int idx = tid; idx < N * lda; idx += G) s.A[idx] = -s.A[idx];
+        __syncthreads();
+        for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + i] += ihg;
+        __syncthreads();
+      }
       bool ok;
       int pstep = -2;
-      if constexpr (NS > 0) {  // compile-time N: rows in registers, implicit pivoting (ck_linalg.cuh)
+      if constexpr (REG_SEG) {  // A = I/(h gamma) - J formed while the rows are loaded into registers
+        double arow[NS > 0 ? NS : 1];
+        if (tid < NS) {
+#pragma unroll
+          for (int j = 0; j < NS; ++j) arow[j] = -s.A[(size_t)tid * lda + j] + (j == tid ? ihg : 0.0);
+        } else {
+#pragma unroll
+          for (int j = 0; j < NS; ++j) arow[j] = 0.0;
+        }
+        ok = lu_factor_rows_seg<(NS > 0 ? NS : 1), G, 9>(arow, pstep, s.A, lda, s.e, s.c.red);
+      } else if constexpr (REG_FULL) {  // compile-time N: rows in registers, implicit pivoting (ck_linalg.cuh)
         double arow[NS];
         if (tid < NS) {
 #pragma unroll
@@ -246,13 +273,18 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const MechDev 
         ok = lu_factor_block<G>(s.A, lda, N, s.piv, s.c.red);
       }
       if (!ok) { status = CK_ST_ZERO_PIVOT; break; }
+      // compact copies of the 4 x 4 diagonal blocks for the blocked stage solves; the derivative chunk arrays are
+      // dead until the next Jacobian (the stage evaluations below run rhs_coop<G, false>)
+      double* const Lb = s.c.dqs;
+      double* const Ub = s.c.dqs + 3 * N;
+      if constexpr (NS < 0 || REG_SEG) lu_compact4<G>(s.A, lda, N, pstep, Lb, Ub);
       long long k2 = clock64();
       ck[2] += k2 - k1;
       TState t;
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 36);
-      else if constexpr (NS < 0) {
+      if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 36);
+      else if constexpr (NS < 0 || REG_SEG) {
         double bb = (tid < N) ? s.f0[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
+        lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u1[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.f0, s.u1); __syncthreads(); }
@@ -260,38 +292,38 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const MechDev 
       ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = fma(a21, s.u1[i], s.y[i]);
       __syncthreads();
-      rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+      rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
       k2 = clock64(); ck[4] += k2 - k3;
       for (int i = tid; i < N; i += G) s.rhs[i] = fma(c21 * ih, s.u1[i], s.ft[i]);
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 36);
-      else if constexpr (NS < 0) {
+      if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 36);
+      else if constexpr (NS < 0 || REG_SEG) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
+        lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u2[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u2); __syncthreads(); }
       k3 = clock64(); ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = s.y[i] + a31 * s.u1[i] + a32 * s.u2[i];
       __syncthreads();
-      rhs_coop<G, false>(m, s.yt, p, s.ft, s.c, t);
+      rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
       k2 = clock64(); ck[4] += k2 - k3;
       c_rhs += 2;
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c31 * s.u1[i] + c32 * s.u2[i]) * ih;
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 36);
-      else if constexpr (NS < 0) {
+      if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 36);
+      else if constexpr (NS < 0 || REG_SEG) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
+        lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u3[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u3); __syncthreads(); }
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c41 * s.u1[i] + c42 * s.u2[i] + c43 * s.u3[i]) * ih;
       __syncthreads();
-      if constexpr (NS > 0) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 36);
-      else if constexpr (NS < 0) {
+      if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 36);
+      else if constexpr (NS < 0 || REG_SEG) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
-        lu_solve_rows_smem<G>(s.A, lda, N, pstep, s.e, bb, s.c.red + 36);
+        lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u4[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u4); __syncthreads(); }
@@ -464,7 +496,7 @@ extern "C" int32_t ck_integrate_ros(const ck_mech* m, int64_t n, double* y, int6
   // that fit one row per thread (K = 9 is config 1); any other size runs the generic shared-memory path
   if (N == 10) rc = launch_ros<32, 1, 10>(m, a, &grid, st);
   else if (N == 15) rc = launch_ros<32, 1, 15>(m, a, &grid, st);
-  else if (N == 54 && getenv("CK_ROS_REG_LU")) rc = launch_ros<64, 2, 54>(m, a, &grid, st);
+  else if (N == 54 && getenv("CK_ROS_REG_LU")) rc = launch_ros<64, 2, 54>(m, a, &grid, st);  // opt-in: measured slower in the kernel
   else if (N <= 32) rc = launch_ros<32, 1, -1>(m, a, &grid, st);
   else if (N <= 64) rc = launch_ros<64, 2, -1>(m, a, &grid, st);
   else if (N <= 128) rc = launch_ros<128, 4, -1>(m, a, &grid, st);
