@@ -180,6 +180,14 @@ def integrator_extras(torch, ck, dev):
                          "simt_efficiency": rep["simt_efficiency"], "waste_p32_static": rep["waste_p32"],
                          "n_failed": rep["n_failed"],
                          "rhs_only_roofline_frac": rep["rhs_evals"] * slots_rhs / (best * 1e-3) / PEAK_SLOTS}
+            # algorithmic FP64-pipe instructions of the whole integration:
+            # every RHS evaluation, an analytic Jacobian at 2.1 RHS, N^3/3 per LU, 4 N^2 per attempt for the four
+            # stage solves, ~20 N per attempt for the stage vectors, error norm and step control
+            Nn = int(y.shape[0])
+            slots = rep["rhs_evals"] * slots_rhs + rep["jac_evals"] * 2.1 * slots_rhs + rep["lu_factor"] * Nn ** 3 / 3.0 \
+                + (4.0 * Nn * Nn if cfg["call"] == "ros" else 0.0) * rep["attempts"] + 20.0 * Nn * rep["attempts"]
+            out[name]["alg_fp64_inst_per_attempt"] = slots / max(rep["attempts"], 1)
+            out[name]["roofline_frac"] = slots / (best * 1e-3) / PEAK_SLOTS
             M.close()
         except Exception as ex:  # integrator not available yet / failed: report, do not hide
             out[name] = {"error": str(ex)[:200]}
