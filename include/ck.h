@@ -142,6 +142,13 @@ int32_t ck_rhs_slots(const ck_mech* m, double* slots);
 /* Measure the FP64 FMA peak of the device with a register-resident DFMA chain (slots/s). */
 int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream);
 
+/* Waste of each SIMD work unit, Eq. 20: W_j = 1 - sum_i N_i / (P max_i N_i) over the P
+ * consecutive reactors of unit j under the static linear reactor -> lane mapping, N_i = attempts of
+ * reactor i = n_accept[i] + n_reject[i] (n_reject may be null).  All pointers are device pointers owned by the
+ * caller; W has ceil(n / P) entries.  The ragged last unit divides by the lanes it has; a unit whose reactors took
+ * no step has W = 0.  P in [1, 1024].  Enqueues on `stream`. */
+int32_t ck_waste(int64_t n, const int32_t* n_accept, const int32_t* n_reject, int32_t P, double* W, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

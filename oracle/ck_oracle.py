@@ -169,3 +169,18 @@ def tableaus():
 
 def max_threads():
     return int(lib().cko_max_threads())
+
+
+def waste(attempts, P):
+    """Eq. 20 written out: for each work unit j of P consecutive reactors (static linear mapping,
+    PAPER.md:363), W_j = 1 - sum_i N_i / (P max_i N_i).  The ragged last unit divides by the lanes it has; a unit whose
+    reactors took no step has W_j = 0 (the readings of include/ck.h).  Plain Python loop, float64.
+    Pins (tests/test_oracle_waste.py): equal counts -> 0, one busy lane of P -> 1 - 1/P, counts 1..P ->
+    1 - (P + 1) / (2 P), invariance under permutation inside a unit and under scaling of all counts, 0 <= W < 1."""
+    a = [int(v) for v in np.asarray(attempts).ravel()]
+    out = []
+    for b in range(0, len(a), P):
+        unit = a[b:b + P]
+        mx = max(unit)
+        out.append(1.0 - float(sum(unit)) / (float(len(unit)) * float(mx)) if mx > 0 else 0.0)
+    return np.array(out, dtype=np.float64)

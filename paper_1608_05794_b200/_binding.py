@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_ros_phase_cycles"):
+                     "ck_fp64_peak", "ck_version", "ck_ros_phase_cycles", "ck_waste"):
             getattr(L, name).restype = C.c_int32
         _lib = L
     return _lib
@@ -199,6 +199,16 @@ class Mechanism:
                   C.byref(rep) if want_report else None, _stream()))
         return dict(y=y, n_accept=na, n_reject=nr, status=st, h_last=hl, report=rep.as_dict() if want_report else None,
                     ws=ws)
+
+    @staticmethod
+    def waste(n_accept, n_reject, P):
+        """Eq. 20 per work unit of width P (static mapping) from device step counts; returns a device tensor."""
+        import torch
+        n = n_accept.numel()
+        W = torch.empty((n + P - 1) // P if P > 0 else 0, dtype=torch.float64, device=n_accept.device)
+        _check(lib().ck_waste(C.c_int64(n), _ptr(n_accept), _ptr(n_reject) if n_reject is not None else None, int(P),
+                              _ptr(W), _stream()))
+        return W
 
     @staticmethod
     def ros_phase_cycles(ws):
