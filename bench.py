@@ -188,6 +188,19 @@ def integrator_extras(torch, ck, dev):
                 + (4.0 * Nn * Nn if cfg["call"] == "ros" else 0.0) * rep["attempts"] + 20.0 * Nn * rep["attempts"]
             out[name]["alg_fp64_inst_per_attempt"] = slots / max(rep["attempts"], 1)
             out[name]["roofline_frac"] = slots / (best * 1e-3) / PEAK_SLOTS
+            # waste study (Eq. 20 and Figs. 9-10): mean and upper decile of
+            # W over the static work units at the paper's four SIMD widths, from this run's step counts (ck_waste)
+            ws_ = {}
+            for P in (4, 8, 16, 32):
+                Wd = M.waste(res["n_accept"], res["n_reject"], P)
+                ws_[str(P)] = {"mean": float(Wd.mean()), "p90": float(torch.quantile(Wd, 0.9))}
+            out[name]["waste_static"] = ws_
+            if name == "C3":  # the same batch in flame order: neighbours need similar step counts
+                _, yf, pf, _ = make_config(name, flame_ordered=True)
+                rf = M.integrate(cfg["call"], torch.from_numpy(yf).to(dev), torch.from_numpy(pf).to(dev), cfg["dt"],
+                                 rtol=cfg["rtol"], atol=cfg["atol"], ws=ws)
+                out[name]["waste_static_flame_ordered"] = {
+                    str(P): {"mean": float(M.waste(rf["n_accept"], rf["n_reject"], P).mean())} for P in (4, 8, 16, 32)}
             M.close()
         except Exception as ex:  # integrator not available yet / failed: report, do not hide
             out[name] = {"error": str(ex)[:200]}
