@@ -312,7 +312,13 @@ __device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int 
 #pragma unroll
         for (int x = 0; x < 8; ++x) row[j + x] = fma(-l, u[x], r[x]);
       }
-      for (; j < N; ++j) row[j] = fma(-l, prow[j], row[j]);
+      if (j < N) {  // ragged tail as ONE predicated block: a scalar loop pays a shared-memory round trip per column
+        double r[8], u[8];
+#pragma unroll
+        for (int x = 0; x < 8; ++x) { r[x] = (j + x < N) ? row[j + x] : 0.0; u[x] = (j + x < N) ? prow[j + x] : 0.0; }
+#pragma unroll
+        for (int x = 0; x < 8; ++x) if (j + x < N) row[j + x] = fma(-l, u[x], r[x]);
+      }
     }
   }
   __syncthreads();
