@@ -440,10 +440,22 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
     int per_sm = 0, sms = 0;
     const int N = m->K + 1;
     CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+    // threads per evicted reactor: the finisher runs the stragglers' serial chains, so its time is the latency of one
+    // cooperative RHS x 6 x the attempts of the slowest reactor; wider CTAs shorten the reaction loop of that RHS
+    const char* cg = getenv("CK_RKF_COOP_G");
+    const int coop_g = cg ? atoi(cg) : 64;
     if (N <= 32) {
       CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
       CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<32>, 32, smem2));
       rkf45_coop_kernel<32><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 32, smem2, st>>>(m->dev, a);
+    } else if (N <= 64 && coop_g == 256) {
+      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<256>, 256, smem2));
+      rkf45_coop_kernel<256><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 256, smem2, st>>>(m->dev, a);
+    } else if (N <= 64 && coop_g == 128) {
+      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<128>, 128, smem2));
+      rkf45_coop_kernel<128><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 128, smem2, st>>>(m->dev, a);
     } else if (N <= 64) {
       CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
       CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<64>, 64, smem2));
