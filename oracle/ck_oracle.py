@@ -14,26 +14,34 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libck_oracle.so")
 _SRC = [os.path.join(_HERE, f) for f in ("ck_oracle_api.cpp", "ck_oracle_chem.hpp", "ck_oracle_solvers.hpp")]
-_lib = None
+_libs = {}
+# "fma": the SAME sources compiled with fused multiply-add contraction (-mfma -ffp-contract=fast): a second correct
+# FP64 execution of the same algorithm that differs from the default build in the last bit of some operations.
+# Used only by the CPU test that justifies DESIGN.md's parity reading P3 (tests/test_oracle_p3.py).
+_VARIANT_FLAGS = {None: [], "fma": ["-mfma", "-ffp-contract=fast"]}
 
 
-def build(force=False):
+def _path(variant):
+    return _LIB_PATH if variant is None else _LIB_PATH.replace(".so", f"_{variant}.so")
+
+
+def build(force=False, variant=None):
     """Compile the oracle: plain g++ -O2, no fast-math."""
-    if not force and os.path.exists(_LIB_PATH) and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(s) for s in _SRC):
-        return _LIB_PATH
-    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-o", _LIB_PATH, _SRC[0]]
+    path = _path(variant)
+    if not force and os.path.exists(path) and all(os.path.getmtime(path) >= os.path.getmtime(s) for s in _SRC):
+        return path
+    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp"] + _VARIANT_FLAGS[variant] + ["-o", path, _SRC[0]]
     subprocess.run(cmd, check=True, cwd=_HERE)
-    return _LIB_PATH
+    return path
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        build()
-        _lib = C.CDLL(_LIB_PATH)
-        _lib.cko_mech_create.restype = C.c_void_p
-        _lib.cko_estimate_h0.restype = C.c_double
-    return _lib
+def lib(variant=None):
+    if variant not in _libs:
+        L = C.CDLL(build(variant=variant))
+        L.cko_mech_create.restype = C.c_void_p
+        L.cko_estimate_h0.restype = C.c_double
+        _libs[variant] = L
+    return _libs[variant]
 
 
 def _p(a, t=C.c_double):
@@ -53,8 +61,8 @@ def _u8(a):
 
 
 class Mech:
-    def __init__(self, d):
-        L = lib()
+    def __init__(self, d, variant=None):
+        L = self._L = lib(variant)
         self.K, self.R, self.E = int(d["n_species"]), int(d["n_reactions"]), int(d["n_elements"])
         self.N = self.K + 1
         keep = self._keep = dict(
@@ -75,7 +83,7 @@ class Mech:
 
     def __del__(self):
         try:
-            lib().cko_mech_free(self.h)
+            self._L.cko_mech_free(self.h)
         except Exception:
             pass
 
@@ -86,26 +94,26 @@ class Mech:
         assert N == self.N and p.shape == (n,)
         f = np.empty_like(y)
         D = np.empty_like(y) if want_scale else None
-        lib().cko_rhs(self.h, C.c_longlong(n), _p(y), C.c_longlong(n), _p(p), _p(f), C.c_longlong(n),
+        self._L.cko_rhs(self.h, C.c_longlong(n), _p(y), C.c_longlong(n), _p(p), _p(f), C.c_longlong(n),
                       _p(D) if want_scale else None, int(prec), int(nthreads))
         return (f, D) if want_scale else f
 
     def rates(self, y1, p):
         y1 = _f64(y1)
         qf = np.empty(self.R); qr = np.empty(self.R); rc = np.empty(2)
-        lib().cko_rates(self.h, _p(y1), C.c_double(p), _p(qf), _p(qr), _p(rc))
+        self._L.cko_rates(self.h, _p(y1), C.c_double(p), _p(qf), _p(qr), _p(rc))
         return qf, qr, rc[0], rc[1]
 
     def thermo(self, k, T):
         out = np.empty(3)
-        lib().cko_thermo(self.h, int(k), C.c_double(T), _p(out))
+        self._L.cko_thermo(self.h, int(k), C.c_double(T), _p(out))
         return out  # cp/R, H/RT, S/R
 
     def jac(self, y1, p, mode=0, h=0.0, rtol=1e-6, atol=1e-10):
         """One state y1[N] -> J[N,N] (row i = d f_i / d y_j). mode 0 complex-step, 1 FD, 2 (J, Jmag)."""
         y1 = _f64(y1)
         J = np.empty((self.N, self.N)); Jm = np.empty((self.N, self.N))
-        lib().cko_jac(self.h, _p(y1), C.c_double(p), int(mode), C.c_double(h), C.c_double(rtol), C.c_double(atol),
+        self._L.cko_jac(self.h, _p(y1), C.c_double(p), int(mode), C.c_double(h), C.c_double(rtol), C.c_double(atol),
                       _p(J), _p(Jm))
         return (J, Jm) if mode == 2 else J
 
@@ -116,7 +124,7 @@ class Mech:
         assert N == self.N
         na = np.zeros(n, np.int32); nr = np.zeros(n, np.int32); st = np.zeros(n, np.int32)
         hl = np.zeros(n); cnt = np.zeros(3, np.int64)
-        lib().cko_integrate(self.h, 0 if solver == "ros" else 1, C.c_longlong(n), _p(y), C.c_longlong(n), _p(p),
+        self._L.cko_integrate(self.h, 0 if solver == "ros" else 1, C.c_longlong(n), _p(y), C.c_longlong(n), _p(p),
                             C.c_double(dt), C.c_double(rtol), C.c_double(atol), int(jac_mode), C.c_double(h0),
                             int(max_steps), _p(na, C.c_int), _p(nr, C.c_int), _p(st, C.c_int), _p(hl),
                             _p(cnt, C.c_longlong), int(nthreads))
@@ -125,11 +133,11 @@ class Mech:
 
     def estimate_h0(self, y1, p, dt, rtol=1e-6, atol=1e-10):
         y1 = _f64(y1)
-        return float(lib().cko_estimate_h0(self.h, _p(y1), C.c_double(p), C.c_double(dt), C.c_double(rtol), C.c_double(atol)))
+        return float(self._L.cko_estimate_h0(self.h, _p(y1), C.c_double(p), C.c_double(dt), C.c_double(rtol), C.c_double(atol)))
 
     def rk4(self, y1, p, dt, nsteps):
         y1 = _f64(y1).copy()
-        lib().cko_rk4(self.h, _p(y1), C.c_double(p), C.c_double(dt), C.c_longlong(nsteps))
+        self._L.cko_rk4(self.h, _p(y1), C.c_double(p), C.c_double(dt), C.c_longlong(nsteps))
         return y1
 
 

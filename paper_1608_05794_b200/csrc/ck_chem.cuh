@@ -210,6 +210,7 @@ struct RateAux {
   double dlnkf_dT, dlnkr_dT;   // temperature derivatives of the rate constants
   double dci_dM;               // d c_i / d [M]_i at constant T   (0 for plain rows)
   double dci_dT;               // d c_i / d T at constant concentrations (falloff rows)
+  double M;                    // [M]_i of a third-body / falloff row (0 for plain rows)
 };
 
 // Rate of progress q_i of regrouped reaction r.  WANT_AUX also fills the derivative pieces.
@@ -225,7 +226,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
   const double T = t.T;
   double kf, kr;
   rate_constants(k, t, kf, kr);
-  double ci = 1.0, dci_dM = 0.0, dci_dT = 0.0;
+  double ci = 1.0, dci_dM = 0.0, dci_dT = 0.0, Mi = 0.0;
   if (TYPE < 0 ? (r >= m.r_tb) : (TYPE >= 1)) {  // third-body / falloff factor c_i (reading G9)
     const int j = r - m.r_tb;
     double M = Ctot;
@@ -239,6 +240,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
       for (int e = __ldg(m.eptr + j), e1 = __ldg(m.eptr + j + 1); e < e1; ++e)
         M = fma(__ldg(m.eval1 + e), C[(size_t)__ldg(m.espec + e) * CS], M);
     }
+    Mi = M;
     if (TYPE < 0 ? (r < m.r_lind) : (TYPE == 1)) {
       ci = M;
       if (WANT_AUX) dci_dM = 1.0;
@@ -300,7 +302,7 @@ __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnC
     aux->kf = kf; aux->kr = kr; aux->ci = ci; aux->pf = pf; aux->pr = pr;
     aux->dlnkf_dT = (beta + Ta * t.invT) * t.invT;
     aux->dlnkr_dT = (kr > 0.0) ? fma(fma(fma(4.0 * c6, T, 3.0 * c5), T, 2.0 * c4), T, c3) + (c1 - c2 * t.invT) * t.invT : 0.0;
-    aux->dci_dM = dci_dM; aux->dci_dT = dci_dT;
+    aux->dci_dM = dci_dM; aux->dci_dT = dci_dT; aux->M = Mi;
   }
   return ci * (kf * pf - kr * pr);
 }

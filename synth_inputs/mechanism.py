@@ -93,7 +93,7 @@ def _cp_target(T, c_lo, c_hi, pw):
     return c_lo + (c_hi - c_lo) * (1.0 - (1.0 - x) ** pw)
 
 
-def _fit_nasa(c_lo, c_hi, pw, hf_over_R, s298_over_R):
+def _fit_nasa(c_lo, c_hi, pw, hf_over_R, s298_over_R, T_MID=T_MID):
     """Two quartic fits of cp/R joined C0/C1 at T_MID; a6,a7 from Hf(298)/R, S(298)/R and continuity."""
     if c_hi - c_lo < 1e-12:  # monatomic: constant cp
         lo = np.array([c_lo, 0, 0, 0, 0], dtype=np.float64)
@@ -103,21 +103,22 @@ def _fit_nasa(c_lo, c_hi, pw, hf_over_R, s298_over_R):
         Tl = np.linspace(T_LOW, T_MID, 71)
         Vl = np.vander(Tl / 1000.0, 5, increasing=True)
         cl, *_ = np.linalg.lstsq(Vl, _cp_target(Tl, c_lo, c_hi, pw), rcond=None)
-        # high range: constrain value and slope at T_MID (x=1): p(x) = v + s (x-1) + (x-1)^2 (d0 + d1 (x-1) + d2 (x-1)^2)
-        v = cl.sum()
-        s = (cl * np.arange(5))[1:].sum()
+        # high range: constrain value and slope at T_MID (x=xm): p(x) = v + s (x-xm) + (x-xm)^2 (d0 + d1 (x-xm) + d2 (x-xm)^2)
+        xm = T_MID / 1000.0
+        v = (cl * xm ** np.arange(5)).sum()
+        s = (cl[1:] * np.arange(1, 5) * xm ** np.arange(4)).sum()
         Th = np.linspace(T_MID, T_HIGH, 201)
-        z = Th / 1000.0 - 1.0
+        z = Th / 1000.0 - xm
         B = np.stack([z**2, z**3, z**4], axis=1)
         rhs = _cp_target(Th, c_lo, c_hi, pw) - v - s * z
         d, *_ = np.linalg.lstsq(B, rhs, rcond=None)
         # expand in powers of x
         pz = np.array([v, s, d[0], d[1], d[2]])  # coefficients in z
         ch = np.zeros(5)
-        for k, ck in enumerate(pz):  # (x-1)^k binomial expansion
+        for k, ck in enumerate(pz):  # (x-xm)^k binomial expansion
             for j in range(k + 1):
                 from math import comb
-                ch[j] += ck * comb(k, j) * (-1.0) ** (k - j)
+                ch[j] += ck * comb(k, j) * (-xm) ** (k - j)
         lo = cl / (1000.0 ** np.arange(5))
         hi = ch / (1000.0 ** np.arange(5))
 
@@ -134,7 +135,7 @@ def _fit_nasa(c_lo, c_hi, pw, hf_over_R, s298_over_R):
     return np.concatenate([lo, [a6_lo, a7_lo]]), np.concatenate([hi, [a6_hi, a7_hi]])
 
 
-def _cp_ok(lo, hi):
+def _cp_ok(lo, hi, T_MID=T_MID):
     Tl = np.arange(T_LOW, T_MID + 1, 10.0)
     Th = np.arange(T_MID, T_HIGH + 1, 10.0)
     cl = sum(lo[i] * Tl**i for i in range(5))
@@ -144,9 +145,11 @@ def _cp_ok(lo, hi):
 
 
 def make_mechanism(n_species, n_reactions, elements, seed, fuel, max_c=2,
-                   n_third=None, n_troe=None, n_lindemann=0, k_cap=3.0e13, k_cap_uni=1.0e10):
-    """Return a dict describing a synthetic mechanism (keys mirror ck_mech_desc)."""
+                   n_third=None, n_troe=None, n_lindemann=0, k_cap=3.0e13, k_cap_uni=1.0e10, t_mid_choices=None, exclude_from_pool=()):
+    """Return a dict describing a synthetic mechanism (keys mirror ck_mech_desc).
+    t_mid_choices: draw each species' NASA range break from this list (own RNG stream; default: 1000 K for all)."""
     rng = np.random.default_rng(seed)
+    rng_tm = np.random.default_rng([seed, 7919])
     elements = list(elements)
     E = len(elements)
     mass = np.array([ATOMIC_MASS[e] for e in elements])
@@ -162,6 +165,9 @@ def make_mechanism(n_species, n_reactions, elements, seed, fuel, max_c=2,
     hf = [a[2] for a in anchors]
     have = {tuple(c) for c in comps}
     cands = [c for c in _candidate_species(elements, max_c, rng) if tuple(c) not in have]
+    if exclude_from_pool:  # e.g. no nitrogen chemistry in a small model (N2 stays as an inert anchor)
+        bad = [elements.index(e) for e in exclude_from_pool]
+        cands = [c for c in cands if not any(c[b] for b in bad)]
     # light species first so that the small H/O radical pool is always present
     cands.sort(key=lambda c: (int(c.sum()), tuple(c)))
     need = n_species - len(comps)
@@ -191,6 +197,9 @@ def make_mechanism(n_species, n_reactions, elements, seed, fuel, max_c=2,
     nasa_hi = np.zeros((K, 7))
     hf_R = np.zeros(K)
     s_R = np.zeros(K)
+    t_mid = np.full(K, T_MID)
+    if t_mid_choices is not None:
+        t_mid = np.asarray(rng_tm.choice(np.asarray(t_mid_choices, dtype=np.float64), size=K), dtype=np.float64)
     for k in range(K):
         hf_R[k] = hf[k] if hf[k] is not None else rng.uniform(-2.5e4, 3.5e4)
         s_R[k] = float(np.clip(18.0 + 2.5 * natoms[k] + rng.uniform(-3, 3), 15.0, 40.0))
@@ -201,14 +210,13 @@ def make_mechanism(n_species, n_reactions, elements, seed, fuel, max_c=2,
             c_hi = min(8.0, c_lo + rng.uniform(0.35, 0.6) * natoms[k])
         for _ in range(100):
             pw = rng.uniform(1.5, 3.0)
-            lo, hi = _fit_nasa(c_lo, c_hi, pw, hf_R[k], s_R[k])
-            if _cp_ok(lo, hi):
+            lo, hi = _fit_nasa(c_lo, c_hi, pw, hf_R[k], s_R[k], float(t_mid[k]))
+            if _cp_ok(lo, hi, float(t_mid[k])):
                 break
             c_hi = c_lo + 0.9 * (c_hi - c_lo)
         else:
             raise RuntimeError("thermo fit failed")
         nasa_lo[k], nasa_hi[k] = lo, hi
-    t_mid = np.full(K, T_MID)
 
     # ---- reactions -----------------------------------------------------------------------
     active = [k for k in range(K) if not inert[k]]
@@ -338,9 +346,139 @@ def make_mechanism(n_species, n_reactions, elements, seed, fuel, max_c=2,
         A0=A0, beta0=beta0, Ea0=Ea0, troe=np.ascontiguousarray(troe),
         eff_ptr=np.array(eff_ptr, dtype=np.int32), eff_spec=np.array(eff_spec, dtype=np.int32),
         eff_val=np.array(eff_val, dtype=np.float64),
-        roles=roles, inert=inert, seed=seed,
+        roles=roles, inert=inert, seed=seed, hf_R=hf_R, s_R=s_R,
     )
     return mech
+
+
+def with_row_kinds(mech, seed, n_lindemann=0, frac_irreversible=0.0, n_termolecular=0, n_both_sides=0,
+                   n_many_eff=0, many_eff=8, split_irreversible=False):
+    """Post-process a generated mechanism so that it holds the reaction kinds the paper's formulation covers but
+    the BASELINE recipes never draw (PAPER.md:113 third-body "and/or pressure effects"; PAPER.md:119 irreversible
+    reactions; Eq. 14 with nu > 1; PAPER.md:149 a model of irreversible reactions only).  Own RNG stream.
+      n_lindemann        Troe rows turned into Lindemann rows (same low-pressure limit, F = 1)
+      frac_irreversible  share of rows marked irreversible (k_r = 0)
+      n_termolecular     appended balanced rows A + B + C <=> D (+E), all species distinct
+      n_both_sides       appended rows 2A + B <=> A + C (nu = 2 and a species on both sides)
+      n_many_eff         third-body / falloff rows given `many_eff` non-unit efficiencies
+      split_irreversible every reversible row becomes TWO irreversible rows, forward and backward, the backward one
+                         with Arrhenius parameters of its own (the shape of an explicit-reverse model)."""
+    rng = np.random.default_rng([int(seed), 104729])
+    K = mech["n_species"]
+    comps, inert = mech["elem_comp"], mech["inert"]
+    hf_R, s_R = mech["hf_R"], mech["s_R"]
+    Rcal = 1.98720425864083
+    rows = []
+    for i in range(mech["n_reactions"]):
+        rs = slice(mech["reac_ptr"][i], mech["reac_ptr"][i + 1]); ps = slice(mech["prod_ptr"][i], mech["prod_ptr"][i + 1])
+        es = slice(mech["eff_ptr"][i], mech["eff_ptr"][i + 1])
+        rows.append(dict(reac=dict(zip(mech["reac_spec"][rs].tolist(), mech["reac_nu"][rs].tolist())),
+                         prod=dict(zip(mech["prod_spec"][ps].tolist(), mech["prod_nu"][ps].tolist())),
+                         A=float(mech["A"][i]), beta=float(mech["beta"][i]), Ea=float(mech["Ea"][i]),
+                         rev=int(mech["reversible"][i]), type=int(mech["type"][i]), A0=float(mech["A0"][i]),
+                         beta0=float(mech["beta0"][i]), Ea0=float(mech["Ea0"][i]), troe=mech["troe"][i].copy(),
+                         eff=dict(zip(mech["eff_spec"][es].tolist(), mech["eff_val"][es].tolist()))))
+    active = [k for k in range(K) if not inert[k]]
+    key = lambda c: tuple(int(x) for x in c)
+
+    def orient(lhs, rhs):
+        dh = sum(hf_R[s] for s in rhs) - sum(hf_R[s] for s in lhs)
+        ds = sum(s_R[s] for s in rhs) - sum(s_R[s] for s in lhs)
+        return (lhs, rhs) if (dh - 1500.0 * ds) <= 0 else (rhs, lhs)
+
+    def draw_rate(cap):
+        for _ in range(10000):
+            a = 10.0 ** rng.uniform(8, 14); b = rng.uniform(-1.5, 2.0); e = rng.uniform(0.0, 50.0e3)
+            if max(a * T**b * np.exp(-e / (Rcal * T)) for T in (800.0, 1500.0, 2500.0)) <= cap:
+                return a, b, e
+        raise RuntimeError("rate draw failed")
+
+    def count(lst):
+        d = {}
+        for s in lst:
+            d[s] = d.get(s, 0) + 1
+        return d
+
+    def new_row(lhs, rhs, cap):
+        a, b, e = draw_rate(cap)
+        return dict(reac=count(lhs), prod=count(rhs), A=a, beta=b, Ea=e, rev=1, type=PLAIN, A0=0.0, beta0=0.0, Ea0=0.0,
+                    troe=np.zeros(4), eff={})
+
+    if n_termolecular:
+        single = {key(comps[a]): a for a in active}
+        pairs = {}
+        for a, b in itertools.combinations(active, 2):
+            pairs.setdefault(key(comps[a] + comps[b]), []).append((a, b))
+        found = []
+        for tr in itertools.combinations(active, 3):
+            ks = key(comps[list(tr)].sum(0))
+            if ks in single and single[ks] not in tr:
+                found.append((tr, (single[ks],)))
+            for pr in pairs.get(ks, []):
+                if not set(pr) & set(tr):
+                    found.append((tr, pr))
+        if len(found) < n_termolecular:
+            raise ValueError(f"only {len(found)} termolecular rows available")
+        for j in rng.choice(len(found), size=n_termolecular, replace=False):
+            lhs, rhs = orient(*found[j])
+            rows.append(new_row(lhs, rhs, 1.0e16 if len(lhs) == 3 else 1.0e10))   # cm^6/mol^2/s scale for A+B+C
+    if n_both_sides:
+        single = {}
+        for a in active:
+            single.setdefault(key(comps[a]), []).append(a)
+        found = []
+        for a, b in itertools.permutations(active, 2):
+            for c in single.get(key(comps[a] + comps[b]), []):
+                found.append(((a, a, b), (a, c)))
+        if len(found) < n_both_sides:
+            raise ValueError(f"only {len(found)} both-sides rows available")
+        for j in rng.choice(len(found), size=n_both_sides, replace=False):
+            lhs, rhs = orient(*found[j])
+            rows.append(new_row(lhs, rhs, 1.0e16 if len(lhs) == 3 else 3.0e13))
+    troe_rows = [i for i, r in enumerate(rows) if r["type"] == TROE]
+    for i in troe_rows[:n_lindemann]:
+        rows[i]["type"] = LINDEMANN
+    special = [i for i, r in enumerate(rows) if r["type"] != PLAIN]
+    for i in special[:n_many_eff]:
+        who = rng.choice(K, size=min(many_eff, K), replace=False)
+        rows[i]["eff"] = {int(s): float(rng.uniform(0.5, 12.0)) for s in sorted(who)}
+    if frac_irreversible > 0:
+        for i in rng.choice(len(rows), size=int(round(frac_irreversible * len(rows))), replace=False):
+            rows[i]["rev"] = 0
+    if split_irreversible:
+        out = []
+        for r in rows:
+            f = dict(r); f["rev"] = 0
+            out.append(f)
+            if r["rev"]:
+                a, b, e = draw_rate(1.0e10 if sum(r["prod"].values()) == 1 else 3.0e13)
+                g = dict(r); g.update(reac=r["prod"], prod=r["reac"], A=a, beta=b, Ea=e, rev=0)
+                if r["type"] >= LINDEMANN:
+                    g["A0"] = a * 10.0 ** rng.uniform(4, 6); g["beta0"] = b - rng.uniform(0, 2); g["Ea0"] = rng.uniform(0.0, 50.0e3)
+                out.append(g)
+        rows = out
+    R = len(rows)
+    i32 = lambda a: np.array(a, dtype=np.int32)
+    rp, rs_, rn, pp, ps_, pn, ep, es_, ev = [0], [], [], [0], [], [], [0], [], []
+    for r in rows:
+        for k, nu in sorted(r["reac"].items()):
+            rs_.append(k); rn.append(nu)
+        rp.append(len(rs_))
+        for k, nu in sorted(r["prod"].items()):
+            ps_.append(k); pn.append(nu)
+        pp.append(len(ps_))
+        for k, v in sorted(r["eff"].items()):
+            es_.append(k); ev.append(v)
+        ep.append(len(es_))
+    out = dict(mech)
+    out.update(n_reactions=R, reac_ptr=i32(rp), reac_spec=i32(rs_), reac_nu=i32(rn), prod_ptr=i32(pp), prod_spec=i32(ps_),
+               prod_nu=i32(pn), A=np.array([r["A"] for r in rows]), beta=np.array([r["beta"] for r in rows]),
+               Ea=np.array([r["Ea"] for r in rows]), reversible=np.array([r["rev"] for r in rows], dtype=np.uint8),
+               type=np.array([r["type"] for r in rows], dtype=np.uint8), A0=np.array([r["A0"] for r in rows]),
+               beta0=np.array([r["beta0"] for r in rows]), Ea0=np.array([r["Ea0"] for r in rows]),
+               troe=np.ascontiguousarray(np.array([r["troe"] for r in rows], dtype=np.float64).reshape(R, 4)),
+               eff_ptr=i32(ep), eff_spec=i32(es_), eff_val=np.array(ev, dtype=np.float64))
+    return out
 
 
 def mech_h2(seed=0):
@@ -356,6 +494,33 @@ def mech_c1(seed=1):
 def mech_c4(seed=2):
     """Config 5: 111 species / 784 reactions, C1-C4 shaped."""
     return make_mechanism(111, 784, ["C", "H", "O", "N", "Ar"], seed, fuel=dict(C=2, H=4), max_c=4)
+
+
+def mech_h2co(seed=3):
+    """Table 1's smallest model shape (H2/CO, 14 species / 38 reactions) over {C,H,O,N,Ar}: CO-rich
+    syngas-like fuel, 4 third-body + 3 Troe rows, one of them turned into a Lindemann row."""
+    m = make_mechanism(14, 38, ["C", "H", "O", "N", "Ar"], seed, fuel=dict(C=1, O=1), max_c=1, n_third=4, n_troe=3,
+                       exclude_from_pool=("N",))
+    return with_row_kinds(m, seed, n_lindemann=1)
+
+
+def mech_c1_irrev(seed=4):
+    """53 species, irreversible reactions only (ref. [20]'s model of 53 species / 634 irreversible
+    reactions): 317 reversible-shaped rows of the methane-air-shaped recipe, each written as a forward and a backward
+    irreversible row with Arrhenius parameters of its own."""
+    m = make_mechanism(53, 317, ["C", "H", "O", "N", "Ar"], seed, fuel=dict(C=1, H=4), max_c=2)
+    return with_row_kinds(m, seed, split_irreversible=True)
+
+
+def mech_rowkinds(n_species=20, n_reactions=48, seed=5, max_c=1, **kw):
+    """Every row kind include/ck.h accepts in one small model: Lindemann rows, irreversible rows, termolecular sides
+    (A + B + C, 2A + B), a species on both sides, third-body rows with 8 efficiencies, three distinct t_mid values."""
+    m = make_mechanism(n_species, n_reactions, ["C", "H", "O", "N", "Ar"], seed, fuel=dict(C=1, O=1) if max_c < 2 else dict(C=1, H=4),
+                       max_c=max_c, n_third=max(3, n_reactions // 10), n_troe=max(4, n_reactions // 10),
+                       t_mid_choices=(900.0, 1000.0, 1400.0), exclude_from_pool=("N",) if n_species < 40 else ())
+    opts = dict(n_lindemann=2, frac_irreversible=0.25, n_termolecular=3, n_both_sides=3, n_many_eff=2)
+    opts.update(kw)
+    return with_row_kinds(m, seed, **opts)
 
 
 def mech_decay(A=1.0e3, reversible=False, dS=0.0):

@@ -25,7 +25,8 @@ def _reactant_product(mech, phi):
     f = roles["fuel"]
     c = comp[f][el.index("C")] if "C" in el else 0
     h = comp[f][el.index("H")]
-    o2_st = c + h / 4.0  # moles O2 per mole fuel (stoichiometric)
+    o = comp[f][el.index("O")] if "O" in el else 0
+    o2_st = c + h / 4.0 - o / 2.0  # moles O2 per mole fuel (stoichiometric; oxygen in the fuel counts)
     X = np.zeros((K, n))
     X[f] = 1.0
     o2 = o2_st / phi

@@ -34,13 +34,18 @@ def _run(oracle, name, n, solver=None, jac_mode=0, flags=0, dt=None, flame=False
         if len(rs) == 0:
             return {}
         t = O.integrate(solver, np.ascontiguousarray(y[:, rs]), np.ascontiguousarray(p[rs]), dt, rtol=1e-9, atol=1e-13,
-                        jac_mode=jac_mode, nthreads=16)
+                        jac_mode=0, nthreads=16)
         return {int(r): t["y"][:, i] for i, r in enumerate(rs)}
     ref["tight"] = tight
     return g, res, ref, mech
 
 
-def _check(g, res, ref, n_species, frac_count=0.05, tight=None):
+def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
+    """fd: ROS4 with the finite-difference Jacobian.  Its columns carry rounding noise eps D / sigma_j (reading G12), which
+    differs between any two correct executions and which the step controller amplifies: the two CPU builds of the oracle
+    already differ by 2 accepted / 6 rejected attempts per reactor (tests/test_oracle_p3.py), so the count slack is 2
+    instead of 1, the batch total of rejected attempts may differ by 10 %, and states are judged by DESIGN.md P3."""
+    slack = 2 if fd else 1
     st = res["status"].cpu().numpy()
     assert np.array_equal(st, ref["status"]) and np.all(st == 0)
     T, To = g[0], ref["y"][0]
@@ -51,6 +56,7 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None):
         assert not bad.any(), (int(bad.sum()), float(np.abs(Y - Yo).max()))
     else:  # DESIGN.md P3
         assert bad.mean() <= 1e-3, float(bad.mean())
+        print("P3 fallback:", int(bad.sum()), "of", bad.size, "entries in", len(np.unique(np.where(bad)[1])), "reactors")
         yt = tight(np.unique(np.where(bad)[1]))
         for r, col in yt.items():
             sc = 1e-6 * np.abs(col) + 1e-10
@@ -60,7 +66,14 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None):
     na = res["n_accept"].cpu().numpy(); nr = res["n_reject"].cpu().numpy()
     assert abs(int(na.sum()) - int(ref["n_accept"].sum())) <= frac_count * ref["n_accept"].sum()
     d = np.abs(na - ref["n_accept"])
-    assert np.all(d <= np.maximum(1, np.ceil(frac_count * ref["n_accept"]))), int(d.max())
+    assert np.all(d <= np.maximum(slack, np.ceil(frac_count * ref["n_accept"]))), int(d.max())
+    # rejected attempts (a third of config 3's work): batch total within 5 %, per reactor within max(1, 5 % of its attempts)
+    # (an accept/reject decision at err ~ 1 flips with the last bit, so one flip per reactor is allowed)
+    att_ref = ref["n_accept"] + ref["n_reject"]
+    assert abs(int(nr.sum()) - int(ref["n_reject"].sum())) <= max((2 if fd else 1) * frac_count * ref["n_reject"].sum(), 1), (int(nr.sum()), int(ref["n_reject"].sum()))
+    d = np.abs(nr - ref["n_reject"])
+    print("n_reject |d| max", int(d.max()), "mean", float(d.mean()), "ref mean", float(ref["n_reject"].mean()))
+    assert np.all(d <= np.maximum(slack, np.ceil(frac_count * att_ref))), int(d.max())
     rep = res["report"]
     assert rep["accepted"] == int(na.sum()) and rep["rejected"] == int(nr.sum())
     assert rep["attempts"] == rep["accepted"] + rep["rejected"] and rep["n_failed"] == 0
@@ -76,8 +89,16 @@ def test_ros_c1_full(oracle):
 
 def test_ros_c1_fd_jacobian(oracle):
     g, res, ref, mech = _run(oracle, "C1", 200, jac_mode=1)
-    rep = _check(g, res, ref, 9)
+    rep = _check(g, res, ref, 9, tight=ref["tight"], fd=True)
     assert rep["rhs_evals"] == (10 + 3) * rep["attempts"] + 2 * 200   # N + 3 per attempt
+
+
+@pytest.mark.parametrize("name,n,N", [("C3", 256, 54), ("C5", 32, 112)])
+def test_ros_fd_jacobian_53_and_111_species(oracle, name, n, N):
+    """ROS4 with the finite-difference Jacobian (N + 3 evaluations per attempt) at N = 54 / 112."""
+    g, res, ref, mech = _run(oracle, name, n, jac_mode=1)
+    rep = _check(g, res, ref, N - 1, tight=ref["tight"], fd=True)
+    assert rep["rhs_evals"] == (N + 3) * rep["attempts"] + 2 * n and rep["jac_evals"] == rep["attempts"]
 
 
 @pytest.mark.parametrize("flame", [False, True])
