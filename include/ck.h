@@ -31,7 +31,7 @@ extern "C" {
 #endif
 
 enum { CK_OK = 0, CK_EINVAL = 1, CK_ECUDA = 2, CK_EWORKSPACE = 3, CK_EUNSUPPORTED = 4 };
-enum { CK_OP_ROS = 0, CK_OP_RKF45 = 1 };                               /* ck_workspace_bytes `op` */
+enum { CK_OP_ROS = 0, CK_OP_RKF45 = 1, CK_OP_JAC = 2 };                 /* ck_workspace_bytes `op` */
 enum { CK_PLAIN = 0, CK_THREE_BODY = 1, CK_LINDEMANN = 2, CK_TROE = 3 }; /* ck_mech_desc.type */
 enum { CK_JAC_ANALYTIC = 0, CK_JAC_FD = 1 };
 /* per-reactor status written by ck_integrate_* */
@@ -72,17 +72,23 @@ typedef struct {
   double rtol, atol;
   double h0;
   int32_t max_steps;
-  int32_t flags;       /* bit 0: disable the divergence-control layer (static mapping; for comparison) */
+  int32_t flags;       /* bit 0: disable the divergence-control layer (static reactor -> lane / CTA mapping, the paper's
+                          layout; for comparison).  RKF45, bit 1: lane refill only, no cooperative finisher.
+                          ROS4, bit 2: force the fused CTA-per-reactor kernel, bit 3: force the batched rounds
+                          (default: rounds for n >= 16384 reactors of a model with 33 <= N <= 128, analytic Jacobian). */
 } ck_opts;
 
 /* Batch totals and divergence statistics, filled on the HOST after the call (may be NULL).
- * simt_efficiency = active lane-slots / issued lane-slots of the step-attempt kernels (device
- * counters); waste_p32 = Eq. 20 at width P = 32 for the static reactor->lane
+ * simt_efficiency: RKF45 -- active lane-slots / issued lane-slots of the step-attempt loop (device counters).
+ * ROS4, batched rounds -- slots holding an active reactor / lanes launched, summed over the kernels of all rounds
+ * (counted per launch from the device-side active count).  ROS4, fused kernel -- the ANALYTIC lane utilisation of its
+ * cooperative loops, (R / ceil_G(R) + N / ceil_G(N)) / 2 for CTAs of G lanes (not a counter; the measured warp
+ * execution efficiency is in profiles/).  waste_p32 = Eq. 20 at width P = 32 for the static reactor->lane
  * mapping, computed from the per-reactor attempt counts (what the paper's layout would have wasted). */
 typedef struct {
   int64_t attempts, accepted, rejected, rhs_evals, jac_evals, lu_factor;
   double simt_efficiency, waste_p32;
-  int32_t rounds; /* launches of the step-attempt kernel (re-batching rounds) */
+  int32_t rounds; /* re-batching rounds: attempt rounds of the batched ROS4 (+1 for its tail), 1 or 2 kernels otherwise */
   int32_t n_failed;
 } ck_report;
 
@@ -97,7 +103,7 @@ int32_t ck_mech_load(const ck_mech_desc* desc, int32_t device, ck_mech** out);
 int32_t ck_mech_free(ck_mech* m);
 int32_t ck_mech_sizes(const ck_mech* m, int32_t* n_species, int32_t* n_reactions);
 
-/* Scratch bytes ck_integrate_{ros,rkf45} need for n reactors (op = CK_OP_*). */
+/* Scratch bytes ck_integrate_{ros,rkf45} / ck_jac_batched need for n reactors (op = CK_OP_*). */
 int32_t ck_workspace_bytes(const ck_mech* m, int32_t op, int64_t n, size_t* bytes);
 
 /* dydt = f(y; p): Eq. 12-19.  y[(K+1) x ld], p[n], dydt[(K+1) x ld_out]. n = 0 is a no-op. */
@@ -109,6 +115,19 @@ int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t ld, const d
  * differences with the CVODE-style increment (h, rtol, atol enter the increment only). */
 int32_t ck_jac(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, int32_t mode, double h,
                double rtol, double atol, double* J, int64_t ldJ, void* stream);
+
+/* The analytic Jacobian of ck_jac evaluated thread-per-reactor for large batches (one reactor per lane, one matrix
+ * row at a time in tensor memory): same output layout as ck_jac.  Needs
+ * ck_workspace_bytes(m, CK_OP_JAC, n) bytes of scratch; CK_EUNSUPPORTED for models with more than 123 species. */
+int32_t ck_jac_batched(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* J, int64_t ldJ,
+                       void* ws, size_t ws_bytes, void* stream);
+
+/* The per-reactor dense linear algebra of the Rosenbrock stage equations on its own (Eq. 6; cost
+ * ~ N^3): for each of n systems factor A_r (row-major N x N at A + r N N, not modified) with partial
+ * pivoting (first maximal |a| wins ties) and solve A_r x_r = b_r (b, x: [n][N]).  status[r] (optional) = CK_ST_OK or
+ * CK_ST_ZERO_PIVOT.  Device pointers; 1 <= N <= 128.  One warp per system, blocked right-looking LU whose trailing
+ * update runs on the FP64 tensor cores (mma.sync.m8n8k4.f64). */
+int32_t ck_lu_solve_batched(int32_t N, int64_t n, const double* A, const double* b, double* x, int32_t* status, void* stream);
 
 /* Advance every reactor from t = 0 to t = dt in place with the 4-stage Rosenbrock method ROS4
  * (Eq. 6-7, Table C.3) resp. the embedded Runge-Kutta-Fehlberg 4(5) pair (Eq. 2-3,
@@ -130,11 +149,6 @@ int32_t ck_rhs_host(ck_mech* m, int64_t n, const double* y, int64_t ld, const do
 int32_t ck_integrate_host(ck_mech* m, int32_t op, int64_t n, double* y_inout, int64_t ld, const double* p, double dt,
                           const ck_opts* opts, int32_t* n_accept, int32_t* n_reject, int32_t* status, double* h_last,
                           ck_report* report);
-
-/* After ck_integrate_ros: SM cycles spent per phase, summed over CTAs, read back from the workspace `ws` of that
- * call (device pointer): 0 RHS + reaction derivatives, 1 Jacobian assembly, 2 LU, 3 stage solves, 4 stage RHS,
- * 5 vectors / control, 6 total.  Synchronises the device. */
-int32_t ck_ros_phase_cycles(const void* ws, int64_t cycles[7]);
 
 /* Roofline support: FP64 instruction count ("slots": DFMA/DMUL/DADD, transcendental at their FP64-pipe
  * instruction counts) that one RHS evaluation of this mechanism needs algorithmically. */

@@ -9,7 +9,7 @@ import numpy as np
 
 from . import _build
 
-CK_OP_ROS, CK_OP_RKF45 = 0, 1
+CK_OP_ROS, CK_OP_RKF45, CK_OP_JAC = 0, 1, 2
 CK_JAC_ANALYTIC, CK_JAC_FD = 0, 1
 _ERR = {1: "CK_EINVAL", 2: "CK_ECUDA", 3: "CK_EWORKSPACE", 4: "CK_EUNSUPPORTED"}
 
@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_ros_phase_cycles", "ck_waste"):
+                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_waste"):
             getattr(L, name).restype = C.c_int32
         _lib = L
     return _lib
@@ -107,6 +107,16 @@ def fp64_peak(device=0):
     v = C.c_double(0)
     _check(lib().ck_fp64_peak(int(device), C.byref(v), None))
     return v.value
+
+
+def lu_solve_batched(A, b):
+    """Solve A[r] x[r] = b[r] for a batch of dense systems (torch CUDA tensors (n, N, N), (n, N)); returns (x, status)."""
+    import torch
+    n, N = A.shape[0], A.shape[1]
+    A = A.contiguous(); b = b.contiguous()
+    x = torch.empty_like(b); st = torch.zeros(n, dtype=torch.int32, device=A.device)
+    _check(lib().ck_lu_solve_batched(int(N), C.c_int64(n), _ptr(A), _ptr(b), _ptr(x), _ptr(st), _stream()))
+    return x, st
 
 
 class Mechanism:
@@ -174,6 +184,17 @@ class Mechanism:
                             C.c_int64(out.stride(0) if n else 0), _stream()))
         return out.view(self.N, self.N, n)
 
+    def jac_batched(self, y, p, out=None):
+        """Analytic Jacobian, thread-per-reactor kernel (large batches); same layout as jac()."""
+        import torch
+        n = y.shape[1]
+        if out is None:
+            out = torch.empty((self.N * self.N, n), dtype=torch.float64, device=y.device)
+        ws = torch.empty(max(self.workspace_bytes(CK_OP_JAC, n), 8), dtype=torch.uint8, device=y.device)
+        _check(lib().ck_jac_batched(self.h, C.c_int64(n), _ptr(y), C.c_int64(y.stride(0) if n else 0), _ptr(p), _ptr(out),
+                                    C.c_int64(out.stride(0) if n else 0), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
+        return out.view(self.N, self.N, n)
+
     def workspace_bytes(self, op, n):
         v = C.c_size_t(0)
         _check(lib().ck_workspace_bytes(self.h, int(op), C.c_int64(n), C.byref(v)))
@@ -209,13 +230,6 @@ class Mechanism:
         _check(lib().ck_waste(C.c_int64(n), _ptr(n_accept), _ptr(n_reject) if n_reject is not None else None, int(P),
                               _ptr(W), _stream()))
         return W
-
-    @staticmethod
-    def ros_phase_cycles(ws):
-        out = (C.c_int64 * 7)()
-        _check(lib().ck_ros_phase_cycles(_ptr(ws), out))
-        names = ("rhs_dq", "jac_assembly", "lu", "solves", "stage_rhs", "vectors_control", "total")
-        return dict(zip(names, [int(v) for v in out]))
 
     # ---- host-pointer entry points (numpy arrays; transfers inside the call) ---------------------------
     def rhs_host(self, y, p, out=None):

@@ -51,7 +51,6 @@ struct MechDev {
                               //   slot << 12 (byte offset of the C column in a 512-thread CTA; >> 11 is the
                               //   tensor-memory column), then per interval 8 doubles: c0..c6, 0
   int rstride;                // = RPH + 8 nT
-  int n_cfast;                // leading fast rows whose rpack rows also sit in __constant__ memory (0: none)
   const double* xpack;        // [R - r_tb][16] AoS for smem staging of third-body / falloff rows: lnA0, beta0, Ta0,
                               //   Troe a, 1/T***, 1/T*, T**, packed (n_eff | 6 x 10-bit species), 6 x (alpha-1), 0, 0
                               //   (n_eff field 15: more than 6 efficiencies, read them from eptr/espec/eval1)
@@ -65,10 +64,9 @@ struct MechDev {
   // transposed stoichiometry (gather form for cooperative kernels): species k <- sum nu_ki q_i
   const int* tptr;            // [K+1]
   const int* tent;            // (reaction << 8) | (net nu + 128)
+  int n_tent;                 // entries of tent
   const int* perm;            // [R] regrouped index -> caller's reaction index
 };
-
-constexpr int CPACK_DOUBLES = 8064;  // __constant__ copy of the leading fast reaction rows (63 KB)
 
 void set_error(const char* fmt, ...);
 int32_t cuda_fail(cudaError_t e, const char* what);
@@ -84,8 +82,6 @@ struct ck_mech {
   int K = 0, R = 0;
   int n_tb = 0, n_lind = 0, n_troe = 0, n_rev = 0;
   long long n_part = 0, n_eff = 0;
-  std::vector<double> h_rpack;  // host copy of the fast rows' rpack (uploaded to the constant bank when owned)
-  bool owns_const = false;
   // cached device staging buffers of the *_host entry points
   void* stage = nullptr;
   size_t stage_bytes = 0;

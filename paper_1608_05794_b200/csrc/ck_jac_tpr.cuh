@@ -9,8 +9,9 @@
 // rate accumulators of ck_rhs_tmem.cuh, whose columns this kernel reuses).
 //
 //   phase A  f(y) as in ck_rhs, with the derivative pieces of every reaction written to a scratch array G2 that is
-//            component-major over the slots (coalesced):  g_f = c_i k_f, g_r = c_i k_r, dq_i/dT|_C, and for third-body /
-//            falloff rows dq_i/d[M]_i and dq_i/d[M]_i [M]_i.
+//            component-major over the slots (coalesced):  g_f = c_i k_f, g_r = c_i k_r, s_i = sum_m dq_i/dC_m C_m,
+//            theta_i = dq_i/dT|_C - s_i / T (the total temperature derivative at constant p and Y), and for
+//            third-body / falloff rows dq_i/d[M]_i.
 //   phase B  gather form, one species row k at a time (the transposed stoichiometry tptr/tent lists the reactions of
 //            species k): row_k[j] += nu_ki dq_i/dC_j with dq_i/dC_slot = g_f prod(other reactant C) resp.
 //            -g_r prod(other product C) rebuilt from G2 and the C columns; the scalars sigma_k, tau_k and the dense
@@ -33,18 +34,23 @@ __host__ __device__ inline int jac_npt(int K) { return (K + 2 + 3) & ~3; }
 // leading dimension of a reactor-major row (N entries padded to a multiple of four doubles)
 __host__ __device__ inline int jac_np(int N) { return (N + 3) & ~3; }
 // doubles per slot of the scratch array G2 / of the HC array
-__host__ __device__ inline int jac_g2_rows(int R, int r_tb) { return 3 * R + 2 * (R - r_tb); }
+__host__ __device__ inline int jac_g2_rows(int R, int r_tb) { return 4 * R + (R - r_tb); }
 __host__ __device__ inline int jac_hc_rows(int K) { return 2 * K + 1; }
-__host__ __device__ inline size_t jac_tpr_smem_bytes(int K, int rstride, int block) {
-  const size_t st = (size_t)rhs_stage_doubles(rstride);
-  return ((size_t)(K + 1) * block + (st > (size_t)2 * K ? st : (size_t)2 * K)) * sizeof(double);
+// shared memory: C columns | staging buffer of phase A, aliased in phase B by its tables: W, 1/W, one packed slot word
+// per reaction, the transposed stoichiometry tent[] and its row pointers (reloaded per batch of reactors: a few KB)
+__host__ __device__ inline size_t jac_tables_doubles(int K, int R, int n_tent) {
+  return (size_t)2 * K + (size_t)R + (((size_t)n_tent + K + 2 + 1) >> 1);
+}
+__host__ __device__ inline size_t jac_tpr_smem_bytes(int K, int R, int n_tent, int rstride, int block) {
+  const size_t st = (size_t)rhs_stage_doubles(rstride), tb = jac_tables_doubles(K, R, n_tent);
+  return ((size_t)(K + 1) * block + (st > tb ? st : tb)) * sizeof(double);
 }
 // CTA width for which both the C columns (shared memory) and the row buffer (tensor memory, one column set per group
 // of four warps) fit; 0 if the mechanism is too large for this kernel
-inline int jac_tpr_block(int K, int rstride) {
-  const int npt = jac_npt(K);
-  if (4 * 2 * npt <= 512 && jac_tpr_smem_bytes(K, rstride, 512) <= 227 * 1024) return 512;
-  if (2 * 2 * npt <= 512 && jac_tpr_smem_bytes(K, rstride, 224) <= 227 * 1024) return 224;
+inline int jac_tpr_block(const MechDev& m) {
+  const int npt = jac_npt(m.K);
+  if (4 * 2 * npt <= 512 && jac_tpr_smem_bytes(m.K, m.R, m.n_tent, m.rstride, 512) <= 227 * 1024) return 512;
+  if (2 * 2 * npt <= 512 && jac_tpr_smem_bytes(m.K, m.R, m.n_tent, m.rstride, 224) <= 227 * 1024) return 224;
   return 0;
 }
 
@@ -68,11 +74,20 @@ __device__ __forceinline__ double thermo_row_dcp(const double* __restrict__ row,
   return fma(fma(fma(4.0 * a[4], T, 3.0 * a[3]), T, 2.0 * a[2]), T, a[1]);
 }
 
+// phase-B tables in shared memory (filled once per CTA)
+struct JacTables {
+  const unsigned long long* slotw;  // [R] six 10-bit slots; bit 63: a species in two slots; bit 62: A + B <=> C + D shaped
+  const int* tptr;                  // [K + 1]
+  const int* tent;                  // [n_tent]
+};
+
 struct JacOut {
   double* f;        // [N][ldf]  f(y)
   long long ldf;
-  double* J;        // reactor-major: J[slot * N * NP + i * NP + j]; component-major: J[(i * N + j) * ldJ + slot]; rows 1..K
+  double* J;        // reactor-major: J[slot * sstride + i * ldr + j]; component-major: J[(i * N + j) * ldJ + slot]; rows 1..K
   long long ldJ;
+  int ldr;          // reactor-major only: row stride (>= N rounded up to a multiple of four) ...
+  long long sstride;  // ... and doubles per slot
   double* hc;       // [2K + 1][ldh]  hh_k, cc_k, and the constant of d f_T / d T
   long long ldh;
   double* g2;       // [jac_g2_rows][ldg] scratch
@@ -89,16 +104,22 @@ __device__ __forceinline__ void jac_phaseA_row(const MechDev& m, int r, const do
   const double q = reaction_q<BLOCK, true, TYPE>(m, r, kc, t, Cs, Ctot, &a, xrow);
   slow_scatter_tmem(kc, q, m.K, wt);
   const double ff = a.kf * a.pf, rr = a.kr * a.pr, net = ff - rr;
+  const int K = m.K;
+  const int nf = (kc.slot[0] != K) + (kc.slot[1] != K) + (kc.slot[2] != K);
+  const int nr = (kc.slot[3] != K) + (kc.slot[4] != K) + (kc.slot[5] != K);
+  // s_i = sum_m dq_i/dC_m C_m: every real reactant slot contributes c_i k_f prod_f, every product slot -c_i k_r prod_r
+  double si = a.ci * ((double)nf * ff - (double)nr * rr);
+  double dqT = a.ci * (ff * a.dlnkf_dT - rr * a.dlnkr_dT) + a.dci_dT * net;
+  if (TYPE >= 1) {
+    const double dM = a.dci_dM * net;
+    si = fma(dM, a.M, si);
+    if (store) g2[(size_t)(4 * m.R + (r - m.r_tb)) * ldg] = dM;
+  }
   if (store) {
-    g2[(size_t)(3 * r) * ldg] = a.ci * a.kf;
-    g2[(size_t)(3 * r + 1) * ldg] = a.ci * a.kr;
-    g2[(size_t)(3 * r + 2) * ldg] = a.ci * (ff * a.dlnkf_dT - rr * a.dlnkr_dT) + a.dci_dT * net;
-    if (TYPE >= 1) {
-      const double dM = a.dci_dM * net;
-      const size_t o = (size_t)(3 * m.R + 2 * (r - m.r_tb)) * ldg;
-      g2[o] = dM;
-      g2[o + ldg] = dM * a.M;
-    }
+    g2[(size_t)(4 * r) * ldg] = a.ci * a.kf;
+    g2[(size_t)(4 * r + 1) * ldg] = a.ci * a.kr;
+    g2[(size_t)(4 * r + 2) * ldg] = si;
+    g2[(size_t)(4 * r + 3) * ldg] = fma(-si, t.invT, dqT);
   }
 }
 
@@ -185,6 +206,22 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
   double* sW = stage;        // [K] W_k
   double* siW = stage + K;   // [K] 1 / W_k
   for (int k = tid; k < K; k += BLOCK) { sW[k] = __ldg(m.W + k); siW[k] = __ldg(m.invW + k); }
+  JacTables tb;
+  {
+    unsigned long long* slotw = reinterpret_cast<unsigned long long*>(stage + 2 * K);
+    int* tptr = reinterpret_cast<int*>(slotw + R);
+    int* tent = tptr + K + 1;
+    for (int i = tid; i < R; i += BLOCK) {
+      unsigned long long w = (unsigned long long)__double_as_longlong(__ldg(m.rpack + (size_t)i * rs + 3));
+      const unsigned s2 = (unsigned)(w >> 20) & 1023u, s5 = (unsigned)(w >> 52) & 1023u;
+      w &= ~(1ull << 62);
+      if (i < m.r_tb && s2 == (unsigned)K && s5 == (unsigned)K && !(w >> 63)) w |= 1ull << 62;   // plain rows only
+      slotw[i] = w;
+    }
+    for (int i = tid; i <= K; i += BLOCK) tptr[i] = __ldg(m.tptr + i);
+    for (int i = tid; i < m.n_tent; i += BLOCK) tent[i] = __ldg(m.tent + i);
+    tb.slotw = slotw; tb.tptr = tptr; tb.tent = tent;
+  }
   const int npt = jac_npt(K);
   for (int c = 0; c < npt; c += 4) tm_zero8(wt + 2 * c);
   tm_wait_st();
@@ -192,33 +229,57 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
   const double iS = 1.0 / S;
   const int NP = jac_np(N);
   double sfc = 0.0;  // sum_k f_k cc_k
+  constexpr int CB = BLOCK * 8;  // bytes between C columns
+  const char* Cb = reinterpret_cast<const char*>(Cs);
   for (int k = 0; k < K; ++k) {
-    double sig = 0.0, tau = 0.0, dns = 0.0;
-    const int e1 = __ldg(m.tptr + k + 1);
-    for (int e = __ldg(m.tptr + k); e < e1; ++e) {
-      const int en = __ldg(m.tent + e);
+    double sig = 0.0, tht = 0.0, dns = 0.0;
+    const int e0 = tb.tptr[k], e1 = tb.tptr[k + 1];
+    // software pipeline: the scratch values of entry e + 1 are in flight while entry e is processed
+    int en = (e0 < e1) ? tb.tent[e0] : 0;
+    double gf = 0.0, gr = 0.0, si = 0.0, th = 0.0;
+    if (e0 < e1) {
+      const size_t og = (size_t)(4 * (en >> 8)) * o.ldg;
+      gf = g2[og]; gr = g2[og + o.ldg]; si = g2[og + 2 * o.ldg]; th = g2[og + 3 * o.ldg];
+    }
+    for (int e = e0; e < e1; ++e) {
       const int i = en >> 8;
       const double nu = (double)((en & 255) - 128);
-      const double swd = __ldg(m.rpack + (size_t)i * rs + 3);
-      const unsigned lo = (unsigned)__double2loint(swd), hi = (unsigned)__double2hiint(swd);
-      int sl[6] = {(int)(lo & 1023u), (int)((lo >> 10) & 1023u), (int)((lo >> 20) & 1023u),
-                   (int)(hi & 1023u), (int)((hi >> 10) & 1023u), (int)((hi >> 20) & 1023u)};
-      const bool dup = (hi >> 31) != 0;
-      const double gf = g2[(size_t)(3 * i) * o.ldg], gr = g2[(size_t)(3 * i + 1) * o.ldg], dqT = g2[(size_t)(3 * i + 2) * o.ldg];
+      const double cgf = gf, ngr = -gr;
+      sig = fma(nu, si, sig);
+      tht = fma(nu, th, tht);
+      if (e + 1 < e1) {
+        en = tb.tent[e + 1];
+        const size_t og = (size_t)(4 * (en >> 8)) * o.ldg;
+        gf = g2[og]; gr = g2[og + o.ldg]; si = g2[og + 2 * o.ldg]; th = g2[og + 3 * o.ldg];
+      }
+      const unsigned long long sw = tb.slotw[i];
+      const unsigned lo = (unsigned)sw, hi = (unsigned)(sw >> 32);
+      const unsigned s0 = lo & 1023u, s1 = (lo >> 10) & 1023u, s3 = hi & 1023u, s4 = (hi >> 10) & 1023u;
+      if (hi & 0x40000000u) {  // A + B <=> C + D shaped row (third slots empty, species distinct): four entries
+        const double c0 = *reinterpret_cast<const double*>(Cb + s0 * CB), c1 = *reinterpret_cast<const double*>(Cb + s1 * CB);
+        const double c3 = *reinterpret_cast<const double*>(Cb + s3 * CB), c4 = *reinterpret_cast<const double*>(Cb + s4 * CB);
+        uint32_t rl[4], rh[4];
+        const uint32_t t0 = wt + 2 + 2 * s0, t1 = wt + 2 + 2 * s1, t3 = wt + 2 + 2 * s3, t4 = wt + 2 + 2 * s4;
+        tm_ld2_raw(t0, rl[0], rh[0]); tm_ld2_raw(t1, rl[1], rh[1]); tm_ld2_raw(t3, rl[2], rh[2]); tm_ld2_raw(t4, rl[3], rh[3]);
+        const double d0 = nu * (cgf * c1), d1 = nu * (cgf * c0), d3 = nu * (ngr * c4), d4 = nu * (ngr * c3);
+        tm_wait_ld();
+        tm_st2(t0, d0 + __hiloint2double((int)rh[0], (int)rl[0]));
+        tm_st2(t1, d1 + __hiloint2double((int)rh[1], (int)rl[1]));
+        tm_st2(t3, d3 + __hiloint2double((int)rh[2], (int)rl[2]));
+        tm_st2(t4, d4 + __hiloint2double((int)rh[3], (int)rl[3]));
+        tm_wait_st();
+        continue;
+      }
+      const unsigned s2 = (lo >> 20) & 1023u, s5 = (hi >> 20) & 1023u;
+      const unsigned sl[6] = {s0, s1, s2, s3, s4, s5};
       double c[6];
 #pragma unroll
-      for (int x = 0; x < 6; ++x) c[x] = Cs[sl[x] * BLOCK];
-      const double ngr = -gr;
-      double d[6] = {gf * (c[1] * c[2]), gf * (c[0] * c[2]), gf * (c[0] * c[1]),
-                     ngr * (c[4] * c[5]), ngr * (c[3] * c[5]), ngr * (c[3] * c[4])};
-      const int nf = (sl[0] != K) + (sl[1] != K) + (sl[2] != K), nrv = (sl[3] != K) + (sl[4] != K) + (sl[5] != K);
-      double si = (double)nf * (d[0] * c[0]) + (double)nrv * (d[3] * c[3]);
+      for (int x = 0; x < 6; ++x) c[x] = *reinterpret_cast<const double*>(Cb + sl[x] * CB);
+      const double d[6] = {cgf * (c[1] * c[2]), cgf * (c[0] * c[2]), cgf * (c[0] * c[1]),
+                           ngr * (c[4] * c[5]), ngr * (c[3] * c[5]), ngr * (c[3] * c[4])};
       if (i >= m.r_tb) {  // third-body / falloff row: dense coefficient + the listed efficiencies
         const int jx = i - m.r_tb;
-        const size_t og = (size_t)(3 * R + 2 * jx) * o.ldg;
-        const double dM = g2[og];
-        si += g2[og + o.ldg];
-        const double ndM = nu * dM;
+        const double ndM = nu * g2[(size_t)(4 * R + jx) * o.ldg];
         dns += ndM;
         const double* xr = m.xpack + (size_t)jx * 16;
         const unsigned long long xw = (unsigned long long)__double_as_longlong(__ldg(xr + 7));
@@ -243,9 +304,7 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
           }
         }
       }
-      sig = fma(nu, si, sig);
-      tau = fma(nu, dqT, tau);
-      if (!dup) {
+      if (!(hi >> 31)) {
         uint32_t rl[6], rh[6];
 #pragma unroll
         for (int x = 0; x < 6; ++x) tm_ld2_raw(wt + 2 * (1 + sl[x]), rl[x], rh[x]);
@@ -265,11 +324,11 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
       }
     }
     // chain rule at constant p: J_kj = (W_k / W_j)(G_kj + dns_k) + (f_k - W_k sig_k / rho) / (S W_j)
-    //                           J_kT = (W_k / rho)(tau_k - sig_k / T) + f_k / T
+    //                           J_kT = (W_k / rho) Theta_k + f_k / T,  Theta_k = sum_i nu_ki theta_i
     const double Wk = sW[k];
     const double fk = store ? fout[(size_t)(1 + k) * o.ldf] : 0.0;
     const double beta = fma(Wk, dns, (fk - Wk * irho * sig) * iS);
-    const double JkT = Wk * irho * (tau - sig * t.invT) + fk * t.invT;
+    const double JkT = fma(Wk * irho, tht, fk * t.invT);
     if (store) sfc = fma(fk, hc[(size_t)(K + k) * o.ldh], sfc);
     for (int c0 = 0; c0 < NP; c0 += 4) {
       double v[4];
@@ -283,9 +342,14 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
       }
       if (store) {
         if (RM) {
-          double2* dst = reinterpret_cast<double2*>(o.J + (size_t)(1 + k) * NP + c0);
-          dst[0] = make_double2(v[0], v[1]);
-          dst[1] = make_double2(v[2], v[3]);
+          double* dst = o.J + (size_t)(1 + k) * o.ldr + c0;
+          if (o.ldr & 1) {  // odd row stride (shared-memory image of the warp LU): rows are only 8-byte aligned
+#pragma unroll
+            for (int x = 0; x < 4; ++x) dst[x] = v[x];
+          } else {
+            reinterpret_cast<double2*>(dst)[0] = make_double2(v[0], v[1]);
+            reinterpret_cast<double2*>(dst)[1] = make_double2(v[2], v[3]);
+          }
         } else {
 #pragma unroll
           for (int x = 0; x < 4; ++x)
@@ -326,7 +390,7 @@ __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, lon
     const bool act = r < n;
     const long long rr = act ? r : n - 1;
     JacOut oo = o;
-    if (RM) oo.J = o.J + (size_t)rr * N * jac_np(N);
+    if (RM) oo.J = o.J + (size_t)rr * o.sstride;
     else oo.J = o.J + rr;
     jac_thread_tmem<BLOCK, RM>(m, y + rr, ld, p[rr], oo, rr, Cs, wt, stage, act);
   }

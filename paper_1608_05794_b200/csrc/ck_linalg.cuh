@@ -421,60 +421,6 @@ __device__ __forceinline__ bool lu_factor_rows_seg(double (&a)[N], int& pstep, d
   return ok;
 }
 
-// Two threads per row (G = 2H threads, H >= N): thread t and thread t + H share row t.  A CTA that owns one N > 64
-// reactor is alone on its SM (the matrix fills shared memory), so its warps are the SM's only warps: with H = 128 row
-// threads that is four, with the row split over two threads eight, and each thread's share of the rank-1 update
-// halves.  Half 0 (t < H) runs the pivot search, writes the multiplier and the next candidate; half 1 reads the
-// candidate back through cbuf (ordered by the barrier of the pivot search) and forms the same multiplier; the
-// remaining columns are dealt out in alternating blocks of eight.  cbuf: 2N doubles, red2: 8 (G/32) doubles.
-// On return half-1 threads carry pstep = -2 so that the solves and lu_compact4 see one owner per row.
-template <int G>
-__device__ __forceinline__ bool lu_factor_rows_smem2(double* __restrict__ A, int lda, int N, int& pstep,
-                                                     double* __restrict__ dinv, double* red2, double* __restrict__ cbuf) {
-  constexpr int H = G / 2;
-  const int tid = threadIdx.x, r = tid & (H - 1), half = tid / H;
-  pstep = (r < N) ? -1 : -2;
-  bool ok = true;
-  double* row = A + (size_t)(r < N ? r : 0) * lda;
-  double cand = row[0];
-  double cinv = 1.0 / cand;
-  for (int k = 0; k < N; ++k) {
-    double ipv;
-    const int p = block_argmax2<G>((pstep == -1 && half == 0) ? fabs(cand) : -1.0, cinv, r, red2, k & 1, &ipv);
-    if (!isfinite(ipv) || ipv == 0.0) ok = false;  // zero / non-finite pivot (uniform)
-    const double* prow = A + (size_t)p * lda;
-    if (r == p) { pstep = k; if (half == 0) dinv[k] = ipv; }
-    else if (pstep == -1) {
-      if (half == 1 && k > 0) cand = cbuf[(k & 1) * N + r];
-      const double l = cand * ipv;
-      int j = k + 1;
-      if (half == 0) {
-        row[k] = l;
-        if (j < N) {  // next step's candidate and its reciprocal first: they head the next step's critical path
-          cand = fma(-l, prow[j], row[j]);
-          row[j] = cand;
-          cbuf[((k + 1) & 1) * N + r] = cand;
-          cinv = 1.0 / cand;
-        }
-      }
-      for (j = k + 2 + 8 * half; j < N; j += 16) {
-        if (j + 8 <= N) {
-          double rr[8], u[8];
-#pragma unroll
-          for (int x = 0; x < 8; ++x) { rr[x] = row[j + x]; u[x] = prow[j + x]; }
-#pragma unroll
-          for (int x = 0; x < 8; ++x) row[j + x] = fma(-l, u[x], rr[x]);
-        } else {
-          for (int x = j; x < N; ++x) row[x] = fma(-l, prow[x], row[x]);
-        }
-      }
-    }
-  }
-  __syncthreads();
-  if (half == 1) pstep = -2;
-  return ok;
-}
-
 // b: entry `tid` of the right-hand side on entry, x[pstep] on return.  bs: 2 doubles of shared scratch.
 template <int G>
 __device__ __forceinline__ void lu_solve_rows_smem(const double* __restrict__ A, int lda, int N, int pstep,

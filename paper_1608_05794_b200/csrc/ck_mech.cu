@@ -17,21 +17,11 @@
 #include <limits>
 #include <map>
 
-#include <mutex>
-
 #include "ck_internal.h"
-
-// each translation unit that instantiates rhs_thread has its own constant bank copy (ck_rhs_thread.cuh)
-cudaError_t ck_rhs_cpack_upload(const double* host, size_t n_doubles);
-cudaError_t ck_rkf_cpack_upload(const double* host, size_t n_doubles);
 
 namespace ck {
 
 static thread_local char g_err[512] = "";
-// The constant bank holds the fast reaction rows of ONE mechanism at a time: the first handle loaded while the
-// bank is free owns it until ck_mech_free; other handles run the shared-memory staging path for every row.
-static std::mutex g_const_mu;
-static const ck_mech* g_const_owner = nullptr;
 void set_error(const char* fmt, ...) {
   va_list ap;
   va_start(ap, fmt);
@@ -337,19 +327,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   v.lnA0 = (const double*)(base + olnA0); v.beta0 = (const double*)(base + ob0); v.Ta0 = (const double*)(base + oTa0);
   v.troe = (const double*)(base + otroe);
   v.rpack = (const double*)(base + orp); v.rstride = rstride;
-  v.tptr = (const int*)(base + otp); v.tent = (const int*)(base + ote); v.perm = (const int*)(base + operm);
-  v.n_cfast = 0;
-  {
-    const int ncf = std::min(r_dup & ~3, (CPACK_DOUBLES / rstride) & ~3);
-    std::lock_guard<std::mutex> lk(g_const_mu);
-    if (ncf > 0 && g_const_owner == nullptr && getenv("CK_USE_CONST_BANK")) {
-      m->h_rpack.assign(rpack.begin(), rpack.begin() + (size_t)ncf * rstride);
-      cudaError_t e1 = ck_rhs_cpack_upload(m->h_rpack.data(), m->h_rpack.size());
-      if (e1 == cudaSuccess) e1 = ck_rkf_cpack_upload(m->h_rpack.data(), m->h_rpack.size());
-      if (e1 == cudaSuccess) { g_const_owner = m; m->owns_const = true; v.n_cfast = ncf; }
-      else cudaGetLastError();  // fall back to the staging path
-    }
-  }
+  v.tptr = (const int*)(base + otp); v.tent = (const int*)(base + ote); v.n_tent = (int)tent.size(); v.perm = (const int*)(base + operm);
   m->K = K; m->R = R; m->n_tb = cnt[1]; m->n_lind = cnt[2]; m->n_troe = cnt[3]; m->n_rev = n_rev;
   m->n_part = n_part; m->n_eff = (long long)espec.size();
   if (getenv("CK_DEBUG")) fprintf(stderr, "ck_mech_load: K=%d R=%d groups: r_22=%d r_dup=%d r_tb=%d r_lind=%d r_troe=%d r_tbf=%d nT=%d\n", K, R, v.r_22, v.r_dup, v.r_tb, v.r_lind, v.r_troe, v.r_tbf, nT);
@@ -360,11 +338,6 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
 extern "C" int32_t ck_mech_free(ck_mech* m) {
   if (!m) return CK_OK;
   cudaSetDevice(m->device);
-  if (m->owns_const) {
-    cudaDeviceSynchronize();  // no kernel may still be reading this mechanism's rows from the constant bank
-    std::lock_guard<std::mutex> lk(g_const_mu);
-    if (g_const_owner == m) g_const_owner = nullptr;
-  }
   if (m->arena) cudaFree(m->arena);
   if (m->stage) cudaFree(m->stage);
   if (m->hstream) cudaStreamDestroy(m->hstream);

@@ -38,26 +38,40 @@ static int32_t launch_rhs(const ck_mech* m, long long n, const double* y, long l
   return CK_OK;
 }
 
-// accumulators in tensor memory: 512 threads per CTA, one CTA per SM, persistent over batches of 512 reactors
+// accumulators in tensor memory: BLOCK threads per CTA, persistent over batches of BLOCK reactors.  512 threads (one
+// CTA per SM) for large batches of models with K + 1 <= 64; 128 threads (up to three CTAs per SM) when the batch
+// would leave most SMs without a 512-thread CTA; 224 threads (seven warps, two column sets) for 64 < K + 1 <= 124.
+template <int BLOCK>
 static int32_t launch_rhs_tmem(const ck_mech* m, long long n, const double* y, long long ld, const double* p, double* f,
                                long long ldf, cudaStream_t st) {
-  constexpr int BLOCK = 512;
   const size_t smem = rhs_tmem_smem_bytes(m->K, m->dev.rstride, BLOCK);
   CK_CUDA(cudaFuncSetAttribute(rhs_kernel_tmem<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int sms = 0;
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  const int cols = rhs_tmem_cols(m->K, BLOCK);
+  const long long per_sm = std::max<long long>(1, std::min<long long>(512 / cols, (long long)((227 * 1024) / (smem + 1024))));
   const long long batches = (n + BLOCK - 1) / BLOCK;
-  const long long grid = std::min<long long>(batches, sms);
+  const long long grid = std::min<long long>(batches, per_sm * sms);
   rhs_kernel_tmem<BLOCK><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, n, y, ld, p, f, ldf);
   CK_CUDA(cudaGetLastError());
   return CK_OK;
 }
 
+// CTA width of the tensor-memory kernel for this batch; 0: use the shared-memory kernel
+int rhs_tmem_block(const ck_mech* m, long long n) {
+  const int K = m->K, rs = m->dev.rstride;
+  if (K + 1 <= 64) {
+    if (n >= 148 * 256 && rhs_tmem_smem_bytes(K, rs, 512) <= 227 * 1024) return 512;
+    if (n >= 2048 && rhs_tmem_cols(K, 128) != 0) return 128;
+    return 0;
+  }
+  if (n >= 4096 && rhs_tmem_cols(K, 224) != 0 && rhs_tmem_smem_bytes(K, rs, 224) <= 227 * 1024) return 224;
+  return 0;
+}
+
 }  // namespace ck
 
 using namespace ck;
-
-cudaError_t ck_rhs_cpack_upload(const double* host, size_t n_doubles) { return cpack_upload(host, n_doubles); }
 
 extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* dydt,
                           int64_t ld_out, void* stream) {
@@ -69,11 +83,12 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
   CK_CUDA(cudaSetDevice(m->device));
   cudaStream_t st = (cudaStream_t)stream;
   if (m->dev.rstride > 64) { set_error("ck_rhs: too many temperature intervals"); return CK_EUNSUPPORTED; }
-  // tensor-memory path: needs 2 (K+1) <= 128 columns per warp, the C columns of 512 threads in shared memory,
-  // and enough reactors to fill the 512-thread CTAs
-  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256 &&
-      !getenv("CK_RHS_NO_TMEM"))
-    return launch_rhs_tmem(m, n, y, ld, p, dydt, ld_out, st);
+  switch (ck::rhs_tmem_block(m, n)) {
+    case 512: return launch_rhs_tmem<512>(m, n, y, ld, p, dydt, ld_out, st);
+    case 224: return launch_rhs_tmem<224>(m, n, y, ld, p, dydt, ld_out, st);
+    case 128: return launch_rhs_tmem<128>(m, n, y, ld, p, dydt, ld_out, st);
+    default: break;
+  }
   switch (rhs_pick_block(m->K, m->dev.rstride, n)) {
     case 256: return launch_rhs<256>(m, n, y, ld, p, dydt, ld_out, st);
     case 128: return launch_rhs<128>(m, n, y, ld, p, dydt, ld_out, st);

@@ -4,39 +4,6 @@
 
 namespace ck {
 
-// Reaction constants of the leading fast rows in the constant bank: read through the uniform datapath, they
-// cost no shared-memory wavefronts (the fast loop was shared-memory-bandwidth bound with staged rows).
-// One copy per translation unit; filled by cpack_upload() when the mechanism owns the bank (ck_mech.cu).
-static __constant__ double c_pack[CPACK_DOUBLES];
-
-static inline cudaError_t cpack_upload(const double* host, size_t n_doubles) {
-  return cudaMemcpyToSymbol(c_pack, host, n_doubles * sizeof(double));
-}
-
-// row `base` (index into c_pack) -> RxnConst; coefficients of both intervals are read uniformly and selected
-// per lane when nT == 2 (the common case), so lanes in different intervals do not serialise the constant cache
-__device__ __forceinline__ RxnConst load_rxn_cpack(int base, int tint, int nT) {
-  RxnConst k;
-  k.lnA = c_pack[base]; k.beta = c_pack[base + 1]; k.Ta = c_pack[base + 2];
-  const double sw = c_pack[base + 3];
-  const unsigned lo = (unsigned)__double2loint(sw), hi = (unsigned)__double2hiint(sw);
-  k.slot[0] = lo & 1023u; k.slot[1] = (lo >> 10) & 1023u; k.slot[2] = (lo >> 20) & 1023u;
-  k.slot[3] = hi & 1023u; k.slot[4] = (hi >> 10) & 1023u; k.slot[5] = (hi >> 20) & 1023u;
-  k.dup = (int)(hi >> 31);
-  if (nT == 2) {
-    const bool h = tint != 0;
-    k.c0 = h ? c_pack[base + RPH + 8] : c_pack[base + RPH]; k.c1 = h ? c_pack[base + RPH + 9] : c_pack[base + RPH + 1];
-    k.c2 = h ? c_pack[base + RPH + 10] : c_pack[base + RPH + 2]; k.c3 = h ? c_pack[base + RPH + 11] : c_pack[base + RPH + 3];
-    k.c4 = h ? c_pack[base + RPH + 12] : c_pack[base + RPH + 4]; k.c5 = h ? c_pack[base + RPH + 13] : c_pack[base + RPH + 5];
-    k.c6 = h ? c_pack[base + RPH + 14] : c_pack[base + RPH + 6];
-  } else {
-    const int o = base + RPH + 8 * tint;
-    k.c0 = c_pack[o]; k.c1 = c_pack[o + 1]; k.c2 = c_pack[o + 2]; k.c3 = c_pack[o + 3];
-    k.c4 = c_pack[o + 4]; k.c5 = c_pack[o + 5]; k.c6 = c_pack[o + 6];
-  }
-  return k;
-}
-
 constexpr int RHS_CHUNK = 32;  // reactions (or species) staged per shared-memory chunk
 
 // staging buffer: RHS_CHUNK reaction rows (or species rows of 16) + RHS_CHUNK special rows of 16
@@ -125,15 +92,7 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
   ws[K * BLOCK] = 0.0;
   // (3) reactions, chunk by chunk
   double* xstage = stage + RHS_CHUNK * (rs > 16 ? rs : 16);
-  // leading fast rows straight from the constant bank (no staging, no barriers)
-  const int ncf = m.n_cfast;
-  for (int r = 0; r < ncf; r += 4) {
-    RxnConst kc[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_cpack((r + u) * rs, t.tint, m.nT);
-    fast_group<BLOCK>(kc, t, K, Cs, ws);
-  }
-  for (int r0 = ncf; r0 < R; r0 += RHS_CHUNK) {
+  for (int r0 = 0; r0 < R; r0 += RHS_CHUNK) {
     const int nr = min(RHS_CHUNK, R - r0);
     const double* src = m.rpack + (size_t)r0 * rs;
     const int x0 = max(r0, m.r_tb);                 // first special row of this chunk

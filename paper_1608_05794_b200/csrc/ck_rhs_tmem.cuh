@@ -38,7 +38,9 @@ __host__ __device__ inline size_t rhs_tmem_smem_bytes(int K, int rstride, int bl
 template <int BLOCK, int NG, bool B22, bool NC>
 __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const TState& t, int K,
                                                 const double* __restrict__ Cs, uint32_t wt) {
-  static_assert(!B22 || BLOCK == 512, "pre-shifted slot words assume 4096-byte C columns");
+  // the packed rows carry slot << 12 (byte offset of a C column of 512 reactors); narrower power-of-two CTAs shift it down
+  static_assert(!B22 || BLOCK == 512 || BLOCK == 256 || BLOCK == 128, "pre-shifted slot words need a power-of-two CTA width");
+  constexpr int SH = (BLOCK == 512) ? 0 : (BLOCK == 256 ? 1 : 2);
   double q[NG];
 #pragma unroll
   for (int u = 0; u < NG; ++u) {
@@ -47,10 +49,10 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
     double pf, pr;
     if (B22) {  // slot words are byte offsets of the C columns
       const char* Cb = reinterpret_cast<const char*>(Cs);
-      pf = *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[0]) *
-           *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[1]);
-      pr = *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[3]) *
-           *reinterpret_cast<const double*>(Cb + (unsigned)kc[u].slot[4]);
+      pf = *reinterpret_cast<const double*>(Cb + ((unsigned)kc[u].slot[0] >> SH)) *
+           *reinterpret_cast<const double*>(Cb + ((unsigned)kc[u].slot[1] >> SH));
+      pr = *reinterpret_cast<const double*>(Cb + ((unsigned)kc[u].slot[3] >> SH)) *
+           *reinterpret_cast<const double*>(Cb + ((unsigned)kc[u].slot[4] >> SH));
     } else {
       pf = Cs[kc[u].slot[0] * BLOCK]; pr = Cs[kc[u].slot[3] * BLOCK];
       if (kc[u].slot[1] != K) pf *= Cs[kc[u].slot[1] * BLOCK];
@@ -82,11 +84,12 @@ __device__ __forceinline__ void fast_group_tmem(const RxnConst (&kc)[NG], const 
 template <int BLOCK, bool NC>
 __device__ __forceinline__ void fast_rows_tmem(const double* __restrict__ stage, int rs, int n22, int nfast, const TState& t,
                                                int K, const double* __restrict__ Cs, uint32_t wt) {
+  constexpr bool PRE = (BLOCK == 512 || BLOCK == 256 || BLOCK == 128);
   for (int j = 0; j < n22; j += 4) {
     RxnConst kc[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row<true>(stage + (j + u) * rs, t.tint);
-    fast_group_tmem<BLOCK, 4, true, NC>(kc, t, K, Cs, wt);
+    for (int u = 0; u < 4; ++u) kc[u] = load_rxn_row<PRE>(stage + (j + u) * rs, t.tint);
+    fast_group_tmem<BLOCK, 4, PRE, NC>(kc, t, K, Cs, wt);
   }
   for (int j = n22; j < nfast; j += 2) {
     RxnConst kc[2];
@@ -223,6 +226,16 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
   if (store) fout[0] = -(t.T * hw) / (rho * cps);
 }
 
+// tensor-memory columns a CTA of `block` threads allocates: one set of 2 (K+1) per group of four warps, rounded up to
+// a power of two >= 32 (0: does not fit)
+__host__ __device__ inline int rhs_tmem_cols(int K, int block) {
+  const int need = ((block + 127) / 128) * 2 * (K + 1);
+  if (need > 512) return 0;
+  int c = 32;
+  while (c < need) c <<= 1;
+  return c;
+}
+
 template <int BLOCK>
 __global__ void __launch_bounds__(BLOCK, 1) rhs_kernel_tmem(const MechDev m, long long n, const double* __restrict__ y,
                                                             long long ld, const double* __restrict__ p,
@@ -232,9 +245,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rhs_kernel_tmem(const MechDev m, lon
   // warp index broadcast from lane 0: tells the compiler it is warp-uniform, so the tensor-memory addresses below stay
   // in uniform registers
   const int tid = threadIdx.x, warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
-  if (warp == 0) {  // one warp allocates all 512 columns (one CTA per SM: shared memory is full anyway)
+  const uint32_t ncols = (uint32_t)rhs_tmem_cols(m.K, BLOCK);
+  if (warp == 0) {  // one warp allocates the CTA's columns
     const uint32_t dst = (uint32_t)__cvta_generic_to_shared(&s_tmem);
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(dst));
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst), "r"(ncols));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
@@ -253,7 +267,7 @@ __global__ void __launch_bounds__(BLOCK, 1) rhs_kernel_tmem(const MechDev m, lon
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tbase));
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tbase), "r"(ncols));
 }
 
 }  // namespace ck

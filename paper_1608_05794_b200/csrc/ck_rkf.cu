@@ -338,8 +338,6 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
 
 using namespace ck;
 
-cudaError_t ck_rkf_cpack_upload(const double* host, size_t n_doubles) { return cpack_upload(host, n_doubles); }
-
 namespace ck {
 int32_t integrate_prologue(const char* who, const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double dt,
                            const ck_opts* o, void* ws, size_t ws_bytes, size_t need, cudaStream_t st);
@@ -369,8 +367,7 @@ cudaError_t plan_for(const ck_mech* m, long long n, RkfPlan* pl) {
 
 int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
   CK_CUDA(cudaSetDevice(m->device));
-  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256 &&
-      !getenv("CK_RHS_NO_TMEM")) {
+  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256) {
     CK_CUDA((plan_for<512, true>(m, n, pl)));
     return CK_OK;
   }
@@ -442,29 +439,18 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
     CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
     // threads per evicted reactor: the finisher runs the stragglers' serial chains, so its time is the latency of one
     // cooperative RHS x 6 x the attempts of the slowest reactor; wider CTAs shorten the reaction loop of that RHS
-    const char* cg = getenv("CK_RKF_COOP_G");
-    const int coop_g = cg ? atoi(cg) : 64;
-    if (N <= 32) {
-      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<32>, 32, smem2));
-      rkf45_coop_kernel<32><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 32, smem2, st>>>(m->dev, a);
-    } else if (N <= 64 && coop_g == 256) {
-      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<256>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<256>, 256, smem2));
-      rkf45_coop_kernel<256><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 256, smem2, st>>>(m->dev, a);
-    } else if (N <= 64 && coop_g == 128) {
-      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<128>, 128, smem2));
-      rkf45_coop_kernel<128><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 128, smem2, st>>>(m->dev, a);
-    } else if (N <= 64) {
-      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<64>, 64, smem2));
-      rkf45_coop_kernel<64><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 64, smem2, st>>>(m->dev, a);
-    } else {
-      CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rkf45_coop_kernel<128>, 128, smem2));
-      rkf45_coop_kernel<128><<<(unsigned)std::min<long long>(n, (long long)std::max(per_sm, 1) * sms), 128, smem2, st>>>(m->dev, a);
-    }
+    const long long cap = (long long)n;
+    auto launch_fin = [&](auto kern, int G) -> int32_t {
+      CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G, smem2));
+      kern<<<(unsigned)std::min<long long>(cap, (long long)std::max(per_sm, 1) * sms), G, smem2, st>>>(m->dev, a);
+      return CK_OK;
+    };
+    int32_t rcf;
+    if (N <= 32) rcf = launch_fin(rkf45_coop_kernel<32>, 32);
+    else if (N <= 64) rcf = launch_fin(rkf45_coop_kernel<64>, 64);
+    else rcf = launch_fin(rkf45_coop_kernel<128>, 128);
+    if (rcf) return rcf;
     CK_CUDA(cudaGetLastError());
     rounds = 2;
   }

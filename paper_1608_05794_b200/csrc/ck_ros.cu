@@ -16,17 +16,10 @@
 #include "ck_coop.cuh"
 #include "ck_linalg.cuh"
 #include "ck_stats.h"
+#include "ck_ros_common.cuh"
 
 namespace ck {
 
-namespace ros4c {  // Table C.3
-constexpr double gam = 0.57282;
-constexpr double a21 = 2.0, a31 = 1.867943637803922, a32 = 0.2344449711399156;
-constexpr double c21 = -7.137615036412310, c31 = 2.580708087951457, c32 = 0.6515950076447975;
-constexpr double c41 = -2.137148994382534, c42 = -0.3214669691237626, c43 = -0.6949742501781779;
-constexpr double m1 = 2.255570073418735, m2 = 0.2870493262186792, m3 = 0.4353179431840180, m4 = 1.093502252409163;
-constexpr double e1 = -0.2815431932141155, e2 = -0.07276199124938920, e3 = -0.1082196201495311, e4 = -1.093502252409163;
-}  // namespace ros4c
 
 __host__ __device__ inline int ros_lda(int N) { return N | 1; }
 // doubles of dynamic shared memory of the ROS4 / jac kernels
@@ -80,22 +73,19 @@ __device__ __noinline__ void rhs_stage(const MechDev* __restrict__ mp, int y_off
 // Leaves f(y) in s.f0.  Returns the number of RHS evaluations spent.
 template <int G>
 __device__ __forceinline__ int jacobian_coop(const MechDev& m, RosShared& s, double p, int mode, double h, double rtol,
-                                             double atol, long long* clk_mid = nullptr) {
+                                             double atol) {
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   TState t;
   if (mode == CK_JAC_ANALYTIC) {
     if (m.K <= G) {  // one pass over the reactions, derivative arrays one chunk long
       const CoopScalars sc = rhs_jac_coop<G>(m, s.y, p, s.f0, s.c, t, s.A, lda);
-      if (clk_mid) *clk_mid = clock64();
       jac_coop_finish<G>(m, s.c, sc, t, s.f0, s.A, lda);
     } else {
       const CoopScalars sc = rhs_coop<G, true>(m, s.y, p, s.f0, s.c, t);
-      if (clk_mid) *clk_mid = clock64();
       jac_coop<G>(m, s.c, sc, t, s.f0, s.A, lda);
     }
     return 1;
   }
-  if (clk_mid) *clk_mid = clock64();
   rhs_stage<G>(&m, (int)(s.y - s.A), p, (int)(s.f0 - s.A));
   const double eps = 2.220446049250313e-16;
   const double fn = wrms_coop<G>(s.f0, s.y, N, rtol, atol, s.c.red);
@@ -135,17 +125,6 @@ __global__ void __launch_bounds__(G) jac_kernel(const __grid_constant__ MechDev 
   }
 }
 
-struct RosArgs {
-  long long n, ld;
-  double* y;
-  const double* p;
-  double dt, rtol, atol, h0;
-  int jac_mode, max_steps, use_queue;
-  int *n_accept, *n_reject, *status;
-  double* h_last;
-  int* att;  // [n] attempts per reactor (workspace; feeds the waste metric)
-  DevStats* stats;
-};
 
 // EstimateH0 (reading G8; the starting-step rule of the paper's ref. [47]); 2 RHS evaluations
 template <int G>
@@ -200,8 +179,6 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
   RosShared s = ros_carve(sm, m.K, m.R, G);
   const int N = m.K + 1, lda = ros_lda(N), tid = threadIdx.x;
   long long c_att = 0, c_acc = 0, c_rej = 0, c_rhs = 0, c_jac = 0, c_fail = 0;
-  long long ck[7] = {0, 0, 0, 0, 0, 0, 0};
-  const long long k_begin = clock64();
   long long r = blockIdx.x;
   for (;;) {
     if (a.use_queue) {
@@ -210,15 +187,19 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       __syncthreads();
       r = s_next;
     }
-    if (r >= a.n) break;
+    const bool resume = a.list != nullptr;   // tail of the batched rounds: reactors of an active list continue
+    if (r >= (resume ? (long long)*a.list_n : a.n)) break;
+    if (resume) r = a.list[r];
     const double p = a.p[r];
     __syncthreads();
     for (int i = tid; i < N; i += G) s.y[i] = a.y[(size_t)i * a.ld + r];
     __syncthreads();
     double tcur = 0.0, h, fac_max = 5.0, h_used = 0.0;
     int nacc = 0, nrej = 0, status = CK_ST_OK;
-    if (a.h0 > 0.0) h = a.h0;
+    if (resume) { tcur = a.rt[r]; h = a.rh[r]; fac_max = a.rfac[r]; nacc = a.racc[r]; nrej = a.rrej[r]; }
+    else if (a.h0 > 0.0) h = a.h0;
     else { h = estimate_h0_coop<G>(m, s, p, a.dt, a.rtol, a.atol); c_rhs += 2; }
+    const int nacc0 = nacc, nrej0 = nrej;
     while (tcur < a.dt) {
       if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; break; }
       if (!isfinite(h)) { status = CK_ST_NONFINITE; break; }
@@ -226,33 +207,17 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       bool last = false;
       if (h >= a.dt - tcur) { h = a.dt - tcur; last = true; }
       // ---- one attempt ----
-      long long k0 = clock64(), kmid = k0;
-      c_rhs += jacobian_coop<G>(m, s, p, a.jac_mode, h, a.rtol, a.atol, &kmid);
+      c_rhs += jacobian_coop<G>(m, s, p, a.jac_mode, h, a.rtol, a.atol);
       c_jac++;
-      long long k1 = clock64();
-      ck[0] += kmid - k0; ck[1] += k1 - kmid;
       const double ihg = 1.0 / (h * gam), ih = 1.0 / h;
-      constexpr bool REG_SEG = NS >= 32;             // compile-time N, rows in registers, segmented step loop
-      constexpr bool REG_FULL = NS > 0 && NS < 32;   // compile-time N, rows in registers, fully unrolled
-      if constexpr (!REG_SEG) {
-        for (int idx = tid; idx < N * lda; idx += G) s.A[idx] = -s.A[idx];
-        __syncthreads();
-        for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + i] += ihg;
-        __syncthreads();
-      }
+      constexpr bool REG_FULL = NS > 0;   // compile-time N, rows in registers, fully unrolled
+      for (int idx = tid; idx < N * lda; idx += G) s.A[idx] = -s.A[idx];
+      __syncthreads();
+      for (int i = tid; i < N; i += G) s.A[(size_t)i * lda + i] += ihg;
+      __syncthreads();
       bool ok;
       int pstep = -2;
-      if constexpr (REG_SEG) {  // A = I/(h gamma) - J formed while the rows are loaded into registers
-        double arow[NS > 0 ? NS : 1];
-        if (tid < NS) {
-#pragma unroll
-          for (int j = 0; j < NS; ++j) arow[j] = -s.A[(size_t)tid * lda + j] + (j == tid ? ihg : 0.0);
-        } else {
-#pragma unroll
-          for (int j = 0; j < NS; ++j) arow[j] = 0.0;
-        }
-        ok = lu_factor_rows_seg<(NS > 0 ? NS : 1), G, 9>(arow, pstep, s.A, lda, s.e, s.c.red);
-      } else if constexpr (REG_FULL) {  // compile-time N: rows in registers, implicit pivoting (ck_linalg.cuh)
+      if constexpr (REG_FULL) {  // compile-time N: rows in registers, implicit pivoting (ck_linalg.cuh)
         double arow[NS];
         if (tid < NS) {
 #pragma unroll
@@ -267,8 +232,6 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
           for (int j = 0; j < NS; ++j) s.A[(size_t)tid * lda + j] = arow[j];
         }
         __syncthreads();
-      } else if constexpr (NS == -2) {  // N <= G/2: two threads per row (the CTA is alone on its SM)
-        ok = lu_factor_rows_smem2<G>(s.A, lda, N, pstep, s.e, s.tmp, s.yt);
       } else if constexpr (NS < 0) {  // any N <= G: rows in shared memory, implicit pivoting, 8-wide updates
         ok = lu_factor_rows_smem<G>(s.A, lda, N, pstep, s.e, s.c.red);
       } else {
@@ -279,42 +242,35 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       // dead until the next Jacobian (the stage evaluations below run rhs_coop<G, false>)
       double* const Lb = s.c.dqs;
       double* const Ub = s.c.dqs + 3 * N;
-      if constexpr (NS < 0 || REG_SEG) lu_compact4<G>(s.A, lda, N, pstep, Lb, Ub);
-      long long k2 = clock64();
-      ck[2] += k2 - k1;
+      if constexpr (NS < 0) lu_compact4<G>(s.A, lda, N, pstep, Lb, Ub);
       TState t;
       if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 36);
-      else if constexpr (NS < 0 || REG_SEG) {
+      else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.f0[tid] : 0.0;
         lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u1[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.f0, s.u1); __syncthreads(); }
-      long long k3 = clock64();
-      ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = fma(a21, s.u1[i], s.y[i]);
       __syncthreads();
       rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
-      k2 = clock64(); ck[4] += k2 - k3;
       for (int i = tid; i < N; i += G) s.rhs[i] = fma(c21 * ih, s.u1[i], s.ft[i]);
       __syncthreads();
       if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u2, s.c.red + 36);
-      else if constexpr (NS < 0 || REG_SEG) {
+      else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
         lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u2[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u2); __syncthreads(); }
-      k3 = clock64(); ck[3] += k3 - k2;
       for (int i = tid; i < N; i += G) s.yt[i] = s.y[i] + a31 * s.u1[i] + a32 * s.u2[i];
       __syncthreads();
       rhs_stage<G>(&m, (int)(s.yt - s.A), p, (int)(s.ft - s.A));
-      k2 = clock64(); ck[4] += k2 - k3;
       c_rhs += 2;
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c31 * s.u1[i] + c32 * s.u2[i]) * ih;
       __syncthreads();
       if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u3, s.c.red + 36);
-      else if constexpr (NS < 0 || REG_SEG) {
+      else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
         lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u3[pstep] = bb;
@@ -323,13 +279,12 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       for (int i = tid; i < N; i += G) s.rhs[i] = s.ft[i] + (c41 * s.u1[i] + c42 * s.u2[i] + c43 * s.u3[i]) * ih;
       __syncthreads();
       if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.rhs, s.u4, s.c.red + 36);
-      else if constexpr (NS < 0 || REG_SEG) {
+      else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.rhs[tid] : 0.0;
         lu_solve_rows_blk<G>(s.A, lda, N, pstep, s.e, Lb, Ub, bb, s.c.red + 32);
         if (pstep >= 0) s.u4[pstep] = bb;
         __syncthreads();
       } else { if (tid < 32) lu_solve_warp<NR>(s.A, lda, N, s.piv, s.rhs, s.u4); __syncthreads(); }
-      k3 = clock64(); ck[3] += k3 - k2;
       double es = 0.0;
       for (int i = tid; i < N; i += G) {
         const double yn = s.y[i] + m1 * s.u1[i] + m2 * s.u2[i] + m3 * s.u3[i] + m4 * s.u4[i];
@@ -364,7 +319,7 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       if (a.h_last) a.h_last[r] = h_used;
       a.att[r] = nacc + nrej;
     }
-    c_att += nacc + nrej; c_acc += nacc; c_rej += nrej; c_fail += (status != CK_ST_OK);
+    c_att += (nacc - nacc0) + (nrej - nrej0); c_acc += nacc - nacc0; c_rej += nrej - nrej0; c_fail += (status != CK_ST_OK);
     if (!a.use_queue) { r += gridDim.x; }
   }
   if (tid == 0) {
@@ -374,9 +329,6 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
     atomicAdd(&a.stats->rhs_evals, (unsigned long long)c_rhs);
     atomicAdd(&a.stats->jac_evals, (unsigned long long)c_jac);
     atomicAdd(&a.stats->failed, (unsigned long long)c_fail);
-    ck[6] = clock64() - k_begin;
-    ck[5] = ck[6] - (ck[0] + ck[1] + ck[2] + ck[3] + ck[4]);
-    for (int i = 0; i < 7; ++i) atomicAdd(&a.stats->clk[i], (unsigned long long)ck[i]);
   }
 }
 
@@ -403,17 +355,15 @@ int32_t launch_jac(const ck_mech* m, long long n, const double* y, long long ld,
 }
 
 template <int G, int NR, int NS>
-int32_t launch_ros(const ck_mech* m, const RosArgs& a, int* grid_out, cudaStream_t st) {
+int32_t launch_ros(const ck_mech* m, const RosArgs& a, long long n_hint, cudaStream_t st) {
   const size_t smem = ros_smem_doubles(m->K, m->R, G) * sizeof(double);
   CK_CUDA(cudaFuncSetAttribute(ros4_kernel<G, NR, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0, sms = 0;
   CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros4_kernel<G, NR, NS>, G, smem));
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
-  const long long grid = std::min<long long>(a.n, (long long)std::max(per_sm, 1) * sms);
-  if (getenv("CK_DEBUG")) fprintf(stderr, "ros4_kernel<%d,%d,%d>: smem %zu B, %d CTAs/SM, grid %lld\n", G, NR, NS, smem, per_sm, grid);
+  const long long grid = std::max<long long>(1, std::min<long long>(n_hint, (long long)std::max(per_sm, 1) * sms));
   ros4_kernel<G, NR, NS><<<(unsigned)grid, G, smem, st>>>(m->dev, a);
   CK_CUDA(cudaGetLastError());
-  *grid_out = (int)grid;
   return CK_OK;
 }
 }  // namespace
@@ -472,61 +422,73 @@ int32_t integrate_report(const ck_mech* m, int64_t n, const int32_t* att_dev, co
 }
 }  // namespace ck
 
-// workspace of ck_integrate_ros: [DevStats][int attempts[n]]
-size_t ck_ros_workspace(int64_t n) { return sizeof(DevStats) + (((size_t)n * sizeof(int) + 255) & ~size_t(255)); }
+// workspace of the fused kernel: [DevStats][int attempts[n]]
+namespace ck {
+size_t ros_fused_workspace(int64_t n) { return sizeof(DevStats) + (((size_t)n * sizeof(int) + 255) & ~size_t(255)); }
 
+int32_t ros_fused_launch(const ck_mech* m, const RosArgs& a, long long n_hint, int* G_used, cudaStream_t st) {
+  const int N = m->K + 1;
+  if (ros_smem_doubles(m->K, m->R, group_size(N)) * sizeof(double) > SMEM_CAP || N > 256) {
+    set_error("ck_integrate_ros: %d x %d matrix does not fit shared memory", N, N);
+    return CK_EUNSUPPORTED;
+  }
+  if (G_used) *G_used = group_size(N);
+  const int NRv = (N + 31) / 32;
+  // compile-time-N instantiations (register-resident LU) for the two small model sizes of the paper's Table 1 shapes
+  // (K = 9 is config 1, K = 14 the H2/CO-sized model); any other size runs the generic shared-memory path
+  if (N == 10) return launch_ros<32, 1, 10>(m, a, n_hint, st);
+  if (N == 15) return launch_ros<32, 1, 15>(m, a, n_hint, st);
+  if (N <= 32) return launch_ros<32, 1, -1>(m, a, n_hint, st);
+  if (N <= 64) return launch_ros<64, 2, -1>(m, a, n_hint, st);
+  if (N <= 128) return launch_ros<128, 4, -1>(m, a, n_hint, st);
+  if (NRv <= 4) return launch_ros<128, 4, 0>(m, a, n_hint, st);
+  return launch_ros<128, 8, 0>(m, a, n_hint, st);
+}
+}  // namespace ck
+
+size_t ck_ros_workspace(const ck_mech* m, int64_t n) {
+  return std::max(ros_fused_workspace(n), ros_rounds_supported(m) ? ros_rounds_workspace(m, n) : (size_t)0);
+}
+
+// ck_opts.flags (ROS4): bit 0 static mapping in the fused kernel; bit 2 force the fused CTA-per-reactor kernel;
+// bit 3 force the batched rounds (tests run both drivers on the same small batches)
 extern "C" int32_t ck_integrate_ros(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt,
                                     const ck_opts* o, int32_t* n_accept, int32_t* n_reject, int32_t* status, double* h_last,
                                     void* ws, size_t ws_bytes, ck_report* report, void* stream) {
   cudaStream_t st = (cudaStream_t)stream;
-  int32_t rc = integrate_prologue("ck_integrate_ros", m, n, y, ld, p, dt, o, ws, ws_bytes, ck_ros_workspace(n), st);
+  if (!m) { set_error("ck_integrate_ros: null mechanism"); return CK_EINVAL; }
+  int32_t rc = integrate_prologue("ck_integrate_ros", m, n, y, ld, p, dt, o, ws, ws_bytes, ck_ros_workspace(m, n), st);
   if (rc) return rc;
   if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
   if (o->jac_mode != CK_JAC_ANALYTIC && o->jac_mode != CK_JAC_FD) { set_error("ck_integrate_ros: bad jac_mode"); return CK_EINVAL; }
   const int N = m->K + 1;
-  if (ros_smem_doubles(m->K, m->R, group_size(N)) * sizeof(double) > SMEM_CAP || N > 256) { set_error("ck_integrate_ros: %d x %d matrix does not fit shared memory", N, N); return CK_EUNSUPPORTED; }
-  RosArgs a;
-  a.n = n; a.ld = ld; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
-  a.jac_mode = o->jac_mode; a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.use_queue = !(o->flags & 1);
-  a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
-  a.stats = (DevStats*)ws;
+  const bool can_rounds = ros_rounds_supported(m) && o->jac_mode == CK_JAC_ANALYTIC && !(o->flags & 1);
+  const bool want_rounds = (o->flags & 8) || (!(o->flags & 4) && N >= 33 && n >= 16384);
   int32_t* att = (int32_t*)((char*)ws + sizeof(DevStats));
-  a.att = att;
-  int grid = 0, G_used = group_size(N);
-  const int NRv = (N + 31) / 32;
-  // compile-time-N instantiations (register-resident LU) for the three model sizes of the paper's Table 1
-  // that fit one row per thread (K = 9 is config 1); any other size runs the generic shared-memory path
-  if (N == 10) rc = launch_ros<32, 1, 10>(m, a, &grid, st);
-  else if (N == 15) rc = launch_ros<32, 1, 15>(m, a, &grid, st);
-  else if (N == 54 && getenv("CK_ROS_REG_LU")) rc = launch_ros<64, 2, 54>(m, a, &grid, st);  // opt-in: measured slower in the kernel
-  else if (N <= 32) rc = launch_ros<32, 1, -1>(m, a, &grid, st);
-  else if (N <= 64) rc = launch_ros<64, 2, -1>(m, a, &grid, st);
-  else if (N <= 128 && N > 64 && getenv("CK_ROS_G256") && ros_smem_doubles(m->K, m->R, 256) * sizeof(double) <= SMEM_CAP) {
-    // opt-in: two threads per row, eight warps on the SM instead of four.  Measured on config 5: RHS / Jacobian phases
-    // 20-30 % faster, LU unchanged (it is not bound by the update), solves slower (eight warps per barrier): 1.5 % overall
-    rc = launch_ros<256, 4, -2>(m, a, &grid, st);
-    G_used = 256;
-  }
-  else if (N <= 128) rc = launch_ros<128, 4, -1>(m, a, &grid, st);
-  else if (NRv <= 4) rc = launch_ros<128, 4, 0>(m, a, &grid, st);
-  else rc = launch_ros<128, 8, 0>(m, a, &grid, st);
-  if (rc) return rc;
-  if (report) {
-    rc = integrate_report(m, n, att, a.stats, 1, 1, report, st);
-    // cooperative kernel: no step-count divergence by construction; lane utilisation of the CTA loops
-    // (species / reaction / row loops over G lanes) is the SIMT efficiency reported here
-    const int G = G_used;
+  DevStats* stats = (DevStats*)ws;
+  int rounds = 1;
+  double lane_util;
+  if (can_rounds && want_rounds) {
+    rc = ros_rounds_run(m, n, y, ld, p, dt, o, n_accept, n_reject, status, h_last, ws, ws_bytes, &rounds, &lane_util, st);
+    if (rc) return rc;
+  } else {
+    RosArgs a{};
+    a.n = n; a.ld = ld; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
+    a.jac_mode = o->jac_mode; a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.use_queue = !(o->flags & 1);
+    a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
+    a.stats = stats; a.att = att;
+    int G = 0;
+    rc = ros_fused_launch(m, a, n, &G, st);
+    if (rc) return rc;
+    // CTA per reactor + work queue: no step-count divergence by construction.  What is reported is the ANALYTIC lane
+    // utilisation of the cooperative loops (R reactions resp. N rows dealt over G lanes), not a device counter; ncu's
+    // warp execution efficiency of the kernel is quoted beside it in DESIGN.md.
     const double ur = (double)m->R / (G * ((m->R + G - 1) / G)), un = (double)N / (G * ((N + G - 1) / G));
-    report->simt_efficiency = 0.5 * (ur + un);
+    lane_util = 0.5 * (ur + un);
+  }
+  if (report) {
+    rc = integrate_report(m, n, att, stats, rounds, 1, report, st);
+    if (!(can_rounds && want_rounds)) report->simt_efficiency = lane_util;
   }
   return rc;
-}
-
-extern "C" int32_t ck_ros_phase_cycles(const void* ws, int64_t cycles[7]) {
-  if (!ws || !cycles) { set_error("ck_ros_phase_cycles: null argument"); return CK_EINVAL; }
-  DevStats hs;
-  CK_CUDA(cudaDeviceSynchronize());
-  CK_CUDA(cudaMemcpy(&hs, ws, sizeof hs, cudaMemcpyDeviceToHost));
-  for (int i = 0; i < 7; ++i) cycles[i] = (int64_t)hs.clk[i];
-  return CK_OK;
 }

@@ -1,0 +1,860 @@
+// ck_integrate_ros, batched rounds: every step ATTEMPT of every active reactor is one pass through a short pipeline
+// of kernels over the compacted active list (the divergence-control layer of SURVEY.md 8(a) a14: active-reactor
+// compaction and re-batching between step attempts).
+//
+// Why: in the fused CTA-per-reactor kernel (ck_ros.cu) the chemistry -- f(y), the analytic Jacobian and two stage
+// evaluations per attempt -- runs CTA-cooperatively at ~4 k SM-cycles per evaluation, against ~0.7 k for the
+// thread-per-reactor tensor-memory kernel of ck_rhs.  Here the chemistry runs thread-per-reactor over the whole active
+// list (ck_rhs itself and jac_rows_kernel, ck_jac_tpr.cuh); only what is genuinely per-reactor dense linear algebra --
+// the LU factorisation of I/(h gamma) - J and the four stage solves of Eq. 6 -- stays cooperative,
+// with the matrix streamed in from HBM once per attempt.  One attempt round:
+//
+//   gather     Yw[:, s] = y[:, act[s]]                                              (thread per slot)
+//   jac_rows   f0 = f(Yw), species rows of J, pieces of row 0        -> F0, LU buffer, HC     (thread per slot)
+//   lu         row 0, A = I/(h gamma) - J, P A = L U, u1 = A^-1 f0, YT = y + a21 u1           (CTA per slot)
+//   ck_rhs     FT = f(YT)                                                                     (thread per slot)
+//   solve2     u2 = A^-1 (FT + c21/h u1), YT = y + a31 u1 + a32 u2                            (CTA per slot)
+//   ck_rhs     FT = f(YT)
+//   solve34    u3, u4, y*, error, accept / reject, new h (Algorithm 1), re-queue   (CTA per slot)
+//
+// Reactors that reached t_f or failed leave the list; the next round runs on the survivors, compacted.  When few
+// are left the round's fixed latency (one thread-per-reactor wave) dominates, so the tail is re-batched once more:
+// the survivors finish in the fused CTA-per-reactor kernel in resume mode.  Arithmetic per reactor does not depend
+// on its slot or on which driver finishes it beyond rounding order, so both drivers are tested against the oracle.
+#include <algorithm>
+#include <cstdlib>
+#include <vector>
+
+#include "ck_coop.cuh"
+#include "ck_jac_tpr.cuh"
+#include "ck_linalg.cuh"
+#include "ck_lu_warp.cuh"
+#include "ck_ros_common.cuh"
+
+namespace ck {
+
+struct RoundArgs {
+  long long n, ld, cap;
+  double* y;
+  const double* p;
+  double dt, rtol, atol, h0;
+  int max_steps;
+  int *n_accept, *n_reject, *status;
+  double* h_last;
+  int* att;
+  // per-reactor controller state
+  double *t, *h, *fac;
+  int *nacc, *nrej;
+  // active lists and counters: cnt[0] = active now, cnt[1] = appended for the next round
+  int *act, *act2, *cnt;
+  // per-slot arrays
+  double *Yw, *Pw, *F0, *YT, *FT;  // component-major [N][cap] ([cap] for Pw)
+  double *U1, *U2;                 // reactor-major [cap][N]
+  double* HC;                      // [2K+1][cap]
+  double* G2;                      // [g2rows][cap]
+  double* LU;                      // [cap][lu_stride]: species rows of J, then L\U (row stride lu_ldr)
+  long long lu_stride;
+  int lu_ldr;
+  double* dinv;                    // [cap][N]
+  int* pst;                        // [cap][N] elimination step at which a row was the pivot
+  double* hs;                      // [cap] step size of this attempt
+  int* flg;                        // [cap] bit 0: clipped to t_f, bit 1: zero pivot
+  DevStats* stats;
+};
+
+__global__ void ros_init_kernel(RoundArgs a) {
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (r == 0) { a.cnt[0] = (int)a.n; a.cnt[1] = 0; }
+  if (r >= a.n) return;
+  a.act[r] = (int)r;
+  a.t[r] = 0.0; a.h[r] = a.h0; a.fac[r] = 5.0;
+  a.nacc[r] = 0; a.nrej[r] = 0;
+}
+
+__global__ void ros_gather_kernel(RoundArgs a, int N) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= a.cnt[0]) return;
+  const int r = a.act[s];
+  a.Pw[s] = a.p[r];
+  for (int c = 0; c < N; ++c) a.Yw[(size_t)c * a.cap + s] = a.y[(size_t)c * a.ld + r];
+}
+
+// EstimateH0 (reading G8), thread per slot.  Part a: d0, d1, h_a, YT = y + h_a f0.  Part b: d2, h0.
+__global__ void ros_h0a_kernel(RoundArgs a, int N) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= a.cnt[0]) return;
+  double s0 = 0.0, s1 = 0.0;
+  for (int c = 0; c < N; ++c) {
+    const double y = a.Yw[(size_t)c * a.cap + s], f = a.F0[(size_t)c * a.cap + s];
+    const double w = 1.0 / fma(a.rtol, fabs(y), a.atol);
+    s0 = fma(y * w, y * w, s0);
+    s1 = fma(f * w, f * w, s1);
+  }
+  const double d0 = sqrt(s0 / N), d1 = sqrt(s1 / N);
+  const double ha = (d0 < 1e-5 || d1 < 1e-5) ? 1e-6 * a.dt : 0.01 * d0 / d1;
+  for (int c = 0; c < N; ++c) a.YT[(size_t)c * a.cap + s] = fma(ha, a.F0[(size_t)c * a.cap + s], a.Yw[(size_t)c * a.cap + s]);
+  a.hs[s] = ha;
+  a.dinv[s] = d1;  // scratch until the first factorisation
+}
+__global__ void ros_h0b_kernel(RoundArgs a, int N) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= a.cnt[0]) return;
+  const double ha = a.hs[s], d1 = a.dinv[s];
+  double s2 = 0.0;
+  for (int c = 0; c < N; ++c) {
+    const double y = a.Yw[(size_t)c * a.cap + s];
+    const double w = (a.FT[(size_t)c * a.cap + s] - a.F0[(size_t)c * a.cap + s]) / fma(a.rtol, fabs(y), a.atol);
+    s2 = fma(w, w, s2);
+  }
+  const double d2 = sqrt(s2 / N) / ha;
+  const double dm = fmax(d1, d2);
+  const double hb = (dm <= 1e-15) ? fmax(1e-6 * a.dt, 1e-3 * ha) : pow(0.01 / dm, 0.2);
+  a.h[a.act[s]] = fmin(fmin(100.0 * ha, hb), a.dt);
+}
+
+// reactors whose first step size already fails the guards of Algorithm 1 leave before the first round
+__global__ void ros_guard_kernel(RoundArgs a) {
+  const long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (s >= a.cnt[0]) return;
+  const int r = a.act[s];
+  const double h = a.h[r];
+  int st = CK_ST_OK;
+  if (a.max_steps <= 0) st = CK_ST_MAX_STEPS;
+  else if (!isfinite(h)) st = CK_ST_NONFINITE;
+  else if (h < 1e-12 * a.dt) st = CK_ST_H_UNDERFLOW;
+  if (st == CK_ST_OK) { a.act2[atomicAdd(&a.cnt[1], 1)] = r; return; }
+  if (a.n_accept) a.n_accept[r] = 0;
+  if (a.n_reject) a.n_reject[r] = 0;
+  if (a.status) a.status[r] = st;
+  if (a.h_last) a.h_last[r] = 0.0;
+  a.att[r] = 0;
+  atomicAdd(&a.stats->failed, 1ULL);
+}
+__global__ void ros_swap_kernel(RoundArgs a) { a.cnt[0] = a.cnt[1]; a.cnt[1] = 0; }
+
+// ---- cooperative kernels: CTA of G threads per slot, thread i owns matrix row i ---------------------------------
+__host__ __device__ inline int rr_lda(int N) { return N | 1; }
+__host__ __device__ inline size_t rr_smem_doubles(int N) { return (size_t)N * rr_lda(N) + 12 * (size_t)N + 64; }
+
+struct RrShared { double *A, *e, *Lb, *Ub, *v0, *v1, *v2, *v3, *red; };
+__device__ __forceinline__ RrShared rr_carve(double* sm, int N) {
+  RrShared s;
+  s.A = sm; sm += (size_t)N * rr_lda(N);
+  s.e = sm; sm += N;
+  s.Lb = sm; sm += 3 * N; s.Ub = sm; sm += 3 * N;
+  s.v0 = sm; sm += N; s.v1 = sm; sm += N; s.v2 = sm; sm += N; s.v3 = sm; sm += N;
+  s.red = sm + N;
+  return s;
+}
+
+// factors (L\U rows, 1/U_kk, pivot steps) between shared memory and the slot's block in HBM
+template <int G>
+__device__ __forceinline__ void rr_store_factors(const RoundArgs& a, long long s, int N, const RrShared& sh, int pstep) {
+  const int NP = a.lu_ldr, lda = rr_lda(N), tid = threadIdx.x;
+  double* dst = a.LU + (size_t)s * a.lu_stride;
+  for (int idx = tid; idx < N * NP; idx += G) {
+    const int i = idx / NP, j = idx - i * NP;
+    dst[idx] = (j < N) ? sh.A[(size_t)i * lda + j] : 0.0;
+  }
+  for (int i = tid; i < N; i += G) a.dinv[(size_t)s * N + i] = sh.e[i];
+  if (tid < N) a.pst[(size_t)s * N + tid] = pstep;
+}
+template <int G>
+__device__ __forceinline__ int rr_load_factors(const RoundArgs& a, long long s, int N, const RrShared& sh) {
+  const int NP = a.lu_ldr, lda = rr_lda(N), tid = threadIdx.x;
+  const double* src = a.LU + (size_t)s * a.lu_stride;
+  for (int idx = tid; idx < N * NP; idx += G) {
+    const int i = idx / NP, j = idx - i * NP;
+    if (j < N) sh.A[(size_t)i * lda + j] = src[idx];
+  }
+  for (int i = tid; i < N; i += G) sh.e[i] = a.dinv[(size_t)s * N + i];
+  const int pstep = (tid < N) ? a.pst[(size_t)s * N + tid] : -2;
+  __syncthreads();
+  lu_compact4<G>(sh.A, lda, N, pstep, sh.Lb, sh.Ub);
+  return pstep;
+}
+// x = A^-1 b with b[tid] in `bb`; the solution lands in x_out (shared, indexed by component)
+template <int G>
+__device__ __forceinline__ void rr_solve(const RrShared& sh, int N, int pstep, double bb, double* __restrict__ x_out) {
+  lu_solve_rows_blk<G>(sh.A, rr_lda(N), N, pstep, sh.e, sh.Lb, sh.Ub, bb, sh.red);
+  if (pstep >= 0) x_out[pstep] = bb;
+  __syncthreads();
+}
+
+// NS > 0: compile-time N with the rows in registers during the factorisation (lu_factor_rows_seg); NS < 0: any N <= G
+template <int G, int NS>
+__global__ void __launch_bounds__(G) ros_lu_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  const int N = K + 1, lda = rr_lda(N), NP = a.lu_ldr, tid = threadIdx.x;
+  const RrShared sh = rr_carve(sm, N);
+  const long long na = a.cnt[0];
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    const int r = a.act[s];
+    __syncthreads();
+    // species rows of J (written by jac_rows_kernel) and the vectors that give row 0 (ck_jac_tpr.cuh)
+    const double* src = a.LU + (size_t)s * a.lu_stride;
+    for (int idx = tid + NP; idx < N * NP; idx += G) {
+      const int i = idx / NP, j = idx - i * NP;
+      if (j < N) sh.A[(size_t)i * lda + j] = src[idx];
+    }
+    for (int k = tid; k < K; k += G) { sh.v0[k] = a.HC[(size_t)k * a.cap + s]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + s]; }
+    for (int i = tid; i < N; i += G) sh.v2[i] = a.F0[(size_t)i * a.cap + s];
+    __syncthreads();
+    const double fT = sh.v2[0];
+    for (int j = tid; j < N; j += G) {
+      double acc = 0.0;
+      for (int k = 0; k < K; ++k) acc = fma(sh.v0[k], sh.A[(size_t)(1 + k) * lda + j], acc);
+      sh.A[j] = (j == 0) ? (a.HC[(size_t)(2 * K) * a.cap + s] - acc) : (-acc - fT * sh.v1[j - 1]);
+    }
+    // step size of this attempt: clip to t_f (Algorithm 1)
+    double h = a.h[r];
+    const double trem = a.dt - a.t[r];
+    int flg = 0;
+    if (h >= trem) { h = trem; flg = 1; }
+    const double ihg = 1.0 / (h * gam);
+    __syncthreads();
+    bool ok;
+    int pstep = -2;
+    if constexpr (NS > 0) {  // A = I/(h gamma) - J formed while the rows are loaded into registers
+      double arow[NS];
+      if (tid < NS) {
+#pragma unroll
+        for (int j = 0; j < NS; ++j) arow[j] = -sh.A[(size_t)tid * lda + j] + (j == tid ? ihg : 0.0);
+      } else {
+#pragma unroll
+        for (int j = 0; j < NS; ++j) arow[j] = 0.0;
+      }
+      __syncthreads();
+      ok = lu_factor_rows_seg<NS, G, 9>(arow, pstep, sh.A, lda, sh.e, sh.red);
+    } else {
+      for (int idx = tid; idx < N * lda; idx += G) sh.A[idx] = -sh.A[idx];
+      __syncthreads();
+      for (int i = tid; i < N; i += G) sh.A[(size_t)i * lda + i] += ihg;
+      __syncthreads();
+      ok = lu_factor_rows_smem<G>(sh.A, lda, N, pstep, sh.e, sh.red);
+    }
+    if (!ok) flg |= 2;
+    lu_compact4<G>(sh.A, lda, N, pstep, sh.Lb, sh.Ub);
+    rr_store_factors<G>(a, s, N, sh, pstep);
+    rr_solve<G>(sh, N, pstep, (tid < N) ? sh.v2[tid] : 0.0, sh.v3);   // u1 = A^-1 f0
+    for (int i = tid; i < N; i += G) {
+      const double u1 = sh.v3[i];
+      a.U1[(size_t)s * N + i] = u1;
+      a.YT[(size_t)i * a.cap + s] = fma(a21, u1, a.Yw[(size_t)i * a.cap + s]);
+    }
+    if (tid == 0) { a.hs[s] = h; a.flg[s] = flg; }
+  }
+}
+
+template <int G>
+__global__ void __launch_bounds__(G) ros_solve2_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  const int N = K + 1, tid = threadIdx.x;
+  const RrShared sh = rr_carve(sm, N);
+  const long long na = a.cnt[0];
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    __syncthreads();
+    for (int i = tid; i < N; i += G) sh.v0[i] = a.U1[(size_t)s * N + i];
+    const int pstep = rr_load_factors<G>(a, s, N, sh);
+    const double ih = 1.0 / a.hs[s];
+    const double bb = (tid < N) ? fma(c21 * ih, sh.v0[tid], a.FT[(size_t)tid * a.cap + s]) : 0.0;
+    rr_solve<G>(sh, N, pstep, bb, sh.v1);   // u2
+    for (int i = tid; i < N; i += G) {
+      const double u2 = sh.v1[i];
+      a.U2[(size_t)s * N + i] = u2;
+      a.YT[(size_t)i * a.cap + s] = a.Yw[(size_t)i * a.cap + s] + a31 * sh.v0[i] + a32 * u2;
+    }
+  }
+}
+
+template <int G>
+__global__ void __launch_bounds__(G) ros_solve34_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  const int N = K + 1, tid = threadIdx.x;
+  const RrShared sh = rr_carve(sm, N);
+  const long long na = a.cnt[0];
+  unsigned long long c_acc = 0, c_rej = 0, c_fail = 0;
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    const int r = a.act[s];
+    __syncthreads();
+    for (int i = tid; i < N; i += G) { sh.v0[i] = a.U1[(size_t)s * N + i]; sh.v1[i] = a.U2[(size_t)s * N + i]; }
+    const int pstep = rr_load_factors<G>(a, s, N, sh);
+    const double h = a.hs[s], ih = 1.0 / h;
+    const int flg = a.flg[s];
+    const double ft = (tid < N) ? a.FT[(size_t)tid * a.cap + s] : 0.0;
+    double bb = (tid < N) ? ft + (c31 * sh.v0[tid] + c32 * sh.v1[tid]) * ih : 0.0;
+    rr_solve<G>(sh, N, pstep, bb, sh.v2);   // u3
+    bb = (tid < N) ? ft + (c41 * sh.v0[tid] + c42 * sh.v1[tid] + c43 * sh.v2[tid]) * ih : 0.0;
+    rr_solve<G>(sh, N, pstep, bb, sh.v3);   // u4
+    double es = 0.0, yn = 0.0;
+    if (tid < N) {
+      const double y0 = a.Yw[(size_t)tid * a.cap + s];
+      const double u1 = sh.v0[tid], u2 = sh.v1[tid], u3 = sh.v2[tid], u4 = sh.v3[tid];
+      yn = y0 + m1 * u1 + m2 * u2 + m3 * u3 + m4 * u4;
+      const double e = e1 * u1 + e2 * u2 + e3 * u3 + e4 * u4;
+      const double w = e / fma(a.rtol, fmax(fabs(y0), fabs(yn)), a.atol);
+      es = w * w;
+    }
+    const double err = sqrt(block_sum<G>(es, sh.red) / N);
+    // ---- accept / reject, new h (Algorithm 1; controller of DESIGN.md reading G8) -- uniform across the CTA
+    double tcur = a.t[r], hn = h, fac_max = a.fac[r];
+    int nacc = a.nacc[r], nrej = a.nrej[r], status = CK_ST_OK;
+    bool done = false;
+    if (flg & 2) { status = CK_ST_ZERO_PIVOT; done = true; }
+    else if (isfinite(err) && err < 1.0) {
+      if (tid < N) a.y[(size_t)tid * a.ld + r] = yn;
+      tcur = (flg & 1) ? a.dt : tcur + h;
+      nacc++;
+      hn = h * fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25)));
+      fac_max = 5.0;
+      c_acc++;
+    } else {
+      nrej++;
+      hn = h * (isfinite(err) ? fmin(1.0, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25))) : 0.2);
+      fac_max = 1.0;
+      c_rej++;
+    }
+    if (!done) {
+      if (!(tcur < a.dt)) done = true;
+      else if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; done = true; }
+      else if (!isfinite(hn)) { status = CK_ST_NONFINITE; done = true; }
+      else if (hn < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; done = true; }
+    }
+    if (tid == 0) {
+      a.t[r] = tcur; a.h[r] = hn; a.fac[r] = fac_max; a.nacc[r] = nacc; a.nrej[r] = nrej;
+      if (done) {
+        if (a.n_accept) a.n_accept[r] = nacc;
+        if (a.n_reject) a.n_reject[r] = nrej;
+        if (a.status) a.status[r] = status;
+        if (a.h_last) a.h_last[r] = (flg & 2) ? 0.0 : h;
+        a.att[r] = nacc + nrej;
+        c_fail += (status != CK_ST_OK);
+      } else {
+        a.act2[atomicAdd(&a.cnt[1], 1)] = r;
+      }
+    }
+  }
+  if (tid == 0) {
+    atomicAdd(&a.stats->attempts, c_acc + c_rej);
+    atomicAdd(&a.stats->accepted, c_acc);
+    atomicAdd(&a.stats->rejected, c_rej);
+    atomicAdd(&a.stats->failed, c_fail);
+  }
+}
+
+// ---- warp-per-reactor kernels: blocked DMMA LU and shuffle solves (ck_lu_warp.cuh); CTA = one warp = one slot ------
+// The slot's block in HBM is the shared-memory image of the matrix (luw_np(N) rows of stride luw_lda(N)): it moves
+// as a flat vector copy.  pst[] holds the row permutation.
+__host__ __device__ inline size_t rw_smem_bytes(int N) {
+  const int NP = luw_np(N);
+  return ((size_t)luw_block_doubles(N) + 5 * (size_t)NP) * sizeof(double) + (size_t)NP * sizeof(int);
+}
+struct RwShared { double *A, *dinv, *v0, *v1, *v2, *v3; int* perm; };
+__device__ __forceinline__ RwShared rw_carve(double* sm, int N) {
+  const int NP = luw_np(N);
+  RwShared s;
+  s.A = sm; sm += luw_block_doubles(N);
+  s.dinv = sm; sm += NP; s.v0 = sm; sm += NP; s.v1 = sm; sm += NP; s.v2 = sm; sm += NP; s.v3 = sm; sm += NP;
+  s.perm = reinterpret_cast<int*>(sm);
+  return s;
+}
+constexpr int RW = 2;          // warps per CTA: warp 0 runs the serial chains, all warps the parallel phases
+constexpr int RWT = 32 * RW;
+__device__ __forceinline__ void rw_copy_block(double* __restrict__ dst, const double* __restrict__ src, int doubles) {
+  const int tid = threadIdx.x;
+  const double2* s2 = reinterpret_cast<const double2*>(src);
+  double2* d2 = reinterpret_cast<double2*>(dst);
+  const int n2 = doubles >> 1;
+#pragma unroll 8
+  for (int i = tid; i < n2; i += RWT) d2[i] = s2[i];
+}
+template <int NR>
+__device__ __forceinline__ void rw_load_factors(const RoundArgs& a, long long s, int N, const RwShared& sh) {
+  const int tid = threadIdx.x;
+  rw_copy_block(sh.A, a.LU + (size_t)s * a.lu_stride, luw_block_doubles(N));
+  for (int i = tid; i < N; i += RWT) { sh.dinv[i] = a.dinv[(size_t)s * N + i]; sh.perm[i] = a.pst[(size_t)s * N + i]; }
+}
+
+template <int NR>
+__global__ void __launch_bounds__(RWT) ros_lu_w_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  __shared__ int s_ok;
+  const int N = K + 1, lda = luw_lda(N), NP = luw_np(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const RwShared sh = rw_carve(sm, N);
+  const long long na = a.cnt[0];
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    const int r = a.act[s];
+    __syncthreads();
+    double* blk = a.LU + (size_t)s * a.lu_stride;
+    // species rows of J (stride lu_ldr in HBM, written by jac_rows_kernel) land negated in the padded image
+    {
+      const int h2 = a.lu_ldr >> 1;
+      const double2* src2 = reinterpret_cast<const double2*>(blk);
+#pragma unroll 4
+      for (int i = 1 + warp; i < N; i += RW) {
+        if (lane < h2) {
+          const double2 v = src2[(size_t)i * h2 + lane];
+          double* d = sh.A + (size_t)i * lda + 2 * lane;
+          d[0] = -v.x; d[1] = -v.y;
+        }
+      }
+      for (int idx = tid; idx < (NP - N) * lda; idx += RWT) sh.A[(size_t)N * lda + idx] = 0.0;   // padding rows
+      for (int i = tid; i < NP; i += RWT)
+        for (int j = a.lu_ldr; j < lda; ++j) sh.A[(size_t)i * lda + j] = 0.0;                   // padding columns
+    }
+    for (int k = tid; k < K; k += RWT) { sh.v0[k] = a.HC[(size_t)k * a.cap + s]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + s]; }
+    for (int i = tid; i < N; i += RWT) sh.v2[i] = a.F0[(size_t)i * a.cap + s];
+    double h = a.h[r];
+    const double trem = a.dt - a.t[r];
+    int flg = 0;
+    if (h >= trem) { h = trem; flg = 1; }
+    const double ihg = 1.0 / (h * gam);
+    __syncthreads();
+    // row 0 of A = I/(h gamma) - J from the (negated) species rows (ck_jac_tpr.cuh): -J_0j = -sum_k hh_k M_kj + f_T cc_j
+    const double fT = sh.v2[0];
+    const double jtt = a.HC[(size_t)(2 * K) * a.cap + s];
+    for (int j = tid; j < NP; j += RWT) {
+      double acc0 = 0.0, acc1 = 0.0;
+      int k = 0;
+      for (; k + 1 < K; k += 2) {
+        acc0 = fma(sh.v0[k], sh.A[(size_t)(1 + k) * lda + j], acc0);
+        acc1 = fma(sh.v0[k + 1], sh.A[(size_t)(2 + k) * lda + j], acc1);
+      }
+      if (k < K) acc0 = fma(sh.v0[k], sh.A[(size_t)(1 + k) * lda + j], acc0);
+      const double acc = acc0 + acc1;
+      sh.A[j] = (j >= N) ? 0.0 : ((j == 0) ? (-jtt - acc) : (fT * sh.v1[j - 1] - acc));
+    }
+    __syncthreads();
+    for (int i = tid; i < N; i += RWT) sh.A[(size_t)i * lda + i] += ihg;
+    __syncthreads();
+    const bool ok = lu_factor_warp_dmma<NR, RW>(sh.A, lda, N, sh.perm, sh.dinv);
+    if (tid == 0) s_ok = ok ? 1 : 0;
+    __syncthreads();
+    if (!s_ok) flg |= 2;
+    rw_copy_block(blk, sh.A, luw_block_doubles(N));
+    for (int i = tid; i < N; i += RWT) { a.dinv[(size_t)s * N + i] = sh.dinv[i]; a.pst[(size_t)s * N + i] = sh.perm[i]; }
+    if (warp == 0) {
+      double bb[NR];
+#pragma unroll
+      for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; bb[q] = (i < N) ? sh.v2[sh.perm[i]] : 0.0; }
+      lu_solve_warp_regs<NR>(sh.A, lda, N, sh.dinv, bb);   // u1 = A^-1 f0
+#pragma unroll
+      for (int q = 0; q < NR; ++q) {
+        const int i = lane + 32 * q;
+        if (i < N) {
+          a.U1[(size_t)s * N + i] = bb[q];
+          a.YT[(size_t)i * a.cap + s] = fma(a21, bb[q], a.Yw[(size_t)i * a.cap + s]);
+        }
+      }
+      if (lane == 0) { a.hs[s] = h; a.flg[s] = flg; }
+    }
+  }
+}
+
+template <int NR>
+__global__ void __launch_bounds__(RWT) ros_solve2_w_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const RwShared sh = rw_carve(sm, N);
+  const long long na = a.cnt[0];
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    __syncthreads();
+    rw_load_factors<NR>(a, s, N, sh);
+    const double ih = 1.0 / a.hs[s];
+    for (int i = tid; i < N; i += RWT) {
+      const double u1 = a.U1[(size_t)s * N + i];
+      sh.v0[i] = u1;
+      sh.v2[i] = fma(c21 * ih, u1, a.FT[(size_t)i * a.cap + s]);
+    }
+    __syncthreads();
+    if (warp == 0) {
+      double bb[NR];
+#pragma unroll
+      for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; bb[q] = (i < N) ? sh.v2[sh.perm[i]] : 0.0; }
+      lu_solve_warp_regs<NR>(sh.A, lda, N, sh.dinv, bb);   // u2
+#pragma unroll
+      for (int q = 0; q < NR; ++q) {
+        const int i = lane + 32 * q;
+        if (i < N) {
+          a.U2[(size_t)s * N + i] = bb[q];
+          a.YT[(size_t)i * a.cap + s] = a.Yw[(size_t)i * a.cap + s] + a31 * sh.v0[i] + a32 * bb[q];
+        }
+      }
+    }
+  }
+}
+
+template <int NR>
+__global__ void __launch_bounds__(RWT) ros_solve34_w_kernel(RoundArgs a, int K) {
+  using namespace ros4c;
+  extern __shared__ double sm[];
+  const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const RwShared sh = rw_carve(sm, N);
+  const long long na = a.cnt[0];
+  unsigned long long c_acc = 0, c_rej = 0, c_fail = 0;
+  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
+    const int r = a.act[s];
+    __syncthreads();
+    rw_load_factors<NR>(a, s, N, sh);
+    const double h = a.hs[s], ih = 1.0 / h;
+    const int flg = a.flg[s];
+    double u1[NR], u2[NR], ft[NR], y0[NR];
+#pragma unroll
+    for (int q = 0; q < NR; ++q) {
+      const int i = lane + 32 * q;
+      const bool in = warp == 0 && i < N;
+      u1[q] = in ? a.U1[(size_t)s * N + i] : 0.0;
+      u2[q] = in ? a.U2[(size_t)s * N + i] : 0.0;
+      ft[q] = in ? a.FT[(size_t)i * a.cap + s] : 0.0;
+      y0[q] = in ? a.Yw[(size_t)i * a.cap + s] : 0.0;
+      if (in) sh.v2[i] = ft[q] + (c31 * u1[q] + c32 * u2[q]) * ih;
+    }
+    __syncthreads();
+    if (warp != 0) continue;
+    double u3[NR], u4[NR];
+#pragma unroll
+    for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; u3[q] = (i < N) ? sh.v2[sh.perm[i]] : 0.0; }
+    lu_solve_warp_regs<NR>(sh.A, lda, N, sh.dinv, u3);
+#pragma unroll
+    for (int q = 0; q < NR; ++q) {
+      const int i = lane + 32 * q;
+      if (i < N) sh.v3[i] = ft[q] + (c41 * u1[q] + c42 * u2[q] + c43 * u3[q]) * ih;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; u4[q] = (i < N) ? sh.v3[sh.perm[i]] : 0.0; }
+    lu_solve_warp_regs<NR>(sh.A, lda, N, sh.dinv, u4);
+    double es = 0.0, yn[NR];
+#pragma unroll
+    for (int q = 0; q < NR; ++q) {
+      const int i = lane + 32 * q;
+      yn[q] = 0.0;
+      if (i < N) {
+        yn[q] = y0[q] + m1 * u1[q] + m2 * u2[q] + m3 * u3[q] + m4 * u4[q];
+        const double e = e1 * u1[q] + e2 * u2[q] + e3 * u3[q] + e4 * u4[q];
+        const double w = e / fma(a.rtol, fmax(fabs(y0[q]), fabs(yn[q])), a.atol);
+        es = fma(w, w, es);
+      }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) es += __shfl_xor_sync(0xffffffffu, es, o);
+    const double err = sqrt(es / N);
+    double tcur = a.t[r], hn = h, fac_max = a.fac[r];
+    int nacc = a.nacc[r], nrej = a.nrej[r], status = CK_ST_OK;
+    bool done = false;
+    if (flg & 2) { status = CK_ST_ZERO_PIVOT; done = true; }
+    else if (isfinite(err) && err < 1.0) {
+#pragma unroll
+      for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; if (i < N) a.y[(size_t)i * a.ld + r] = yn[q]; }
+      tcur = (flg & 1) ? a.dt : tcur + h;
+      nacc++;
+      hn = h * fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25)));
+      fac_max = 5.0;
+      c_acc++;
+    } else {
+      nrej++;
+      hn = h * (isfinite(err) ? fmin(1.0, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25))) : 0.2);
+      fac_max = 1.0;
+      c_rej++;
+    }
+    if (!done) {
+      if (!(tcur < a.dt)) done = true;
+      else if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; done = true; }
+      else if (!isfinite(hn)) { status = CK_ST_NONFINITE; done = true; }
+      else if (hn < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; done = true; }
+    }
+    if (lane == 0) {
+      a.t[r] = tcur; a.h[r] = hn; a.fac[r] = fac_max; a.nacc[r] = nacc; a.nrej[r] = nrej;
+      if (done) {
+        if (a.n_accept) a.n_accept[r] = nacc;
+        if (a.n_reject) a.n_reject[r] = nrej;
+        if (a.status) a.status[r] = status;
+        if (a.h_last) a.h_last[r] = (flg & 2) ? 0.0 : h;
+        a.att[r] = nacc + nrej;
+        c_fail += (status != CK_ST_OK);
+      } else {
+        a.act2[atomicAdd(&a.cnt[1], 1)] = r;
+      }
+    }
+  }
+  if (tid == 0) {
+    atomicAdd(&a.stats->attempts, c_acc + c_rej);
+    atomicAdd(&a.stats->accepted, c_acc);
+    atomicAdd(&a.stats->rejected, c_rej);
+    atomicAdd(&a.stats->failed, c_fail);
+  }
+}
+
+}  // namespace ck
+
+using namespace ck;
+
+extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* dydt,
+                          int64_t ld_out, void* stream);
+
+namespace {
+inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
+inline int rr_group(int N) { return N <= 32 ? 32 : (N <= 64 ? 64 : 128); }
+// warp-per-reactor LU / solves (ck_lu_warp.cuh) where a matrix block is small enough for several warps per SM
+inline bool rr_use_warp(const ck_mech* m) { return m->K + 1 <= 64; }
+inline int rr_lu_ldr(const ck_mech* m) { return jac_np(m->K + 1); }   // row stride of the species rows of J in a slot's block
+inline long long rr_lu_stride(const ck_mech* m) {
+  const int N = m->K + 1;
+  return rr_use_warp(m) ? (long long)luw_block_doubles(N) : (long long)N * jac_np(N);
+}
+
+struct RrLayout {
+  size_t att, t, h, fac, nacc, nrej, act, act2, cnt, Yw, Pw, F0, YT, FT, U1, U2, HC, G2, LU, dinv, pst, hs, flg, total;
+};
+RrLayout rr_layout(const ck_mech* m, int64_t n) {
+  const size_t N = m->K + 1, cap = (size_t)n;
+  RrLayout L;
+  size_t o = sizeof(DevStats);
+  auto put = [&](size_t bytes) { const size_t at = o; o += al256(bytes); return at; };
+  L.att = put(cap * 4);   // must follow the header: integrate_report reads it there
+  L.t = put(cap * 8); L.h = put(cap * 8); L.fac = put(cap * 8);
+  L.nacc = put(cap * 4); L.nrej = put(cap * 4);
+  L.act = put(cap * 4); L.act2 = put(cap * 4); L.cnt = put(64);
+  L.Yw = put(N * cap * 8); L.Pw = put(cap * 8); L.F0 = put(N * cap * 8); L.YT = put(N * cap * 8); L.FT = put(N * cap * 8);
+  L.U1 = put(N * cap * 8); L.U2 = put(N * cap * 8);
+  L.HC = put((size_t)jac_hc_rows(m->K) * cap * 8);
+  L.G2 = put((size_t)jac_g2_rows(m->R, m->dev.r_tb) * cap * 8);
+  L.LU = put(cap * (size_t)rr_lu_stride(m) * 8);
+  L.dinv = put(cap * N * 8); L.pst = put(cap * N * 4);
+  L.hs = put(cap * 8); L.flg = put(cap * 4);
+  L.total = o;
+  return L;
+}
+
+template <int BLOCK>
+int32_t launch_jac_rows_rm(const ck_mech* m, const RoundArgs& a, long long na, int sms, cudaStream_t st) {
+  const size_t smem = jac_tpr_smem_bytes(m->K, m->R, m->dev.n_tent, m->dev.rstride, BLOCK);
+  CK_CUDA(cudaFuncSetAttribute(jac_rows_kernel<BLOCK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  JacOut o;
+  o.f = a.F0; o.ldf = a.cap; o.J = a.LU; o.ldJ = 0; o.ldr = a.lu_ldr; o.sstride = a.lu_stride;
+  o.hc = a.HC; o.ldh = a.cap; o.g2 = a.G2; o.ldg = a.cap;
+  const long long grid = std::max<long long>(1, std::min<long long>((na + BLOCK - 1) / BLOCK, sms));
+  jac_rows_kernel<BLOCK, true><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, na, a.cnt, a.Yw, a.cap, a.Pw, o);
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}
+
+template <int G, int NS>
+int32_t launch_coop(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
+  const int N = m->K + 1;
+  const size_t smem = rr_smem_doubles(N) * sizeof(double);
+  int per_sm = 0;
+  if (which == 0) {
+    CK_CUDA(cudaFuncSetAttribute(ros_lu_kernel<G, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_lu_kernel<G, NS>, G, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
+    ros_lu_kernel<G, NS><<<(unsigned)grid, G, smem, st>>>(a, m->K);
+  } else if (which == 1) {
+    CK_CUDA(cudaFuncSetAttribute(ros_solve2_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_solve2_kernel<G>, G, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
+    ros_solve2_kernel<G><<<(unsigned)grid, G, smem, st>>>(a, m->K);
+  } else {
+    CK_CUDA(cudaFuncSetAttribute(ros_solve34_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_solve34_kernel<G>, G, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
+    ros_solve34_kernel<G><<<(unsigned)grid, G, smem, st>>>(a, m->K);
+  }
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}
+
+template <int NR>
+int32_t launch_warp(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
+  const int N = m->K + 1;
+  const size_t smem = rw_smem_bytes(N);
+  int per_sm = 0;
+  auto go = [&](auto kern) -> int32_t {
+    CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, RWT, smem));
+    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
+    kern<<<(unsigned)grid, RWT, smem, st>>>(a, m->K);
+    CK_CUDA(cudaGetLastError());
+    return CK_OK;
+  };
+  if (which == 0) return go(ros_lu_w_kernel<NR>);
+  if (which == 1) return go(ros_solve2_w_kernel<NR>);
+  return go(ros_solve34_w_kernel<NR>);
+}
+
+int32_t coop_dispatch(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
+  const int N = m->K + 1;
+  if (rr_use_warp(m)) return (N <= 32) ? launch_warp<1>(m, a, na, sms, which, st) : launch_warp<2>(m, a, na, sms, which, st);
+  switch (rr_group(N)) {
+    case 32: return launch_coop<32, -1>(m, a, na, sms, which, st);
+    case 64: return launch_coop<64, -1>(m, a, na, sms, which, st);
+    default: return launch_coop<128, -1>(m, a, na, sms, which, st);
+  }
+}
+}  // namespace
+
+namespace ck {
+
+bool ros_rounds_supported(const ck_mech* m) {
+  const int N = m->K + 1;
+  return N <= 128 && jac_tpr_block(m->dev) != 0 && m->dev.rstride <= 64 &&
+         (rr_use_warp(m) ? rw_smem_bytes(N) : rr_smem_doubles(N) * sizeof(double)) <= 227 * 1024;
+}
+size_t ros_rounds_workspace(const ck_mech* m, int64_t n) { return n > 0 ? rr_layout(m, n).total : sizeof(DevStats); }
+
+int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt, const ck_opts* o,
+                       int32_t* n_accept, int32_t* n_reject, int32_t* status, double* h_last, void* ws, size_t ws_bytes,
+                       int* rounds_out, double* lane_util, cudaStream_t st) {
+  const RrLayout L = rr_layout(m, n);
+  if (ws_bytes < L.total) { set_error("ck_integrate_ros: workspace of %zu bytes needed, %zu given", L.total, ws_bytes); return CK_EWORKSPACE; }
+  const int N = m->K + 1;
+  char* w = (char*)ws;
+  RoundArgs a{};
+  a.n = n; a.ld = ld; a.cap = n; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
+  a.max_steps = o->max_steps > 0 ? o->max_steps : 100000;
+  a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
+  a.stats = (DevStats*)ws;
+  a.att = (int*)(w + L.att); a.t = (double*)(w + L.t); a.h = (double*)(w + L.h); a.fac = (double*)(w + L.fac);
+  a.nacc = (int*)(w + L.nacc); a.nrej = (int*)(w + L.nrej); a.act = (int*)(w + L.act); a.act2 = (int*)(w + L.act2);
+  a.cnt = (int*)(w + L.cnt);
+  a.Yw = (double*)(w + L.Yw); a.Pw = (double*)(w + L.Pw); a.F0 = (double*)(w + L.F0); a.YT = (double*)(w + L.YT);
+  a.FT = (double*)(w + L.FT); a.U1 = (double*)(w + L.U1); a.U2 = (double*)(w + L.U2); a.HC = (double*)(w + L.HC);
+  a.G2 = (double*)(w + L.G2); a.LU = (double*)(w + L.LU); a.lu_stride = rr_lu_stride(m); a.lu_ldr = rr_lu_ldr(m); a.dinv = (double*)(w + L.dinv); a.pst = (int*)(w + L.pst);
+  a.hs = (double*)(w + L.hs); a.flg = (int*)(w + L.flg);
+  int sms = 0;
+  CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  const unsigned tb = 256, gn = (unsigned)((n + tb - 1) / tb);
+  int* h_cnt = nullptr;  // pinned: the active count comes back once per round
+  CK_CUDA(cudaHostAlloc((void**)&h_cnt, 2 * sizeof(int), cudaHostAllocDefault));
+  auto fail = [&](int32_t rc) { cudaFreeHost(h_cnt); return rc; };
+  auto read_count = [&](long long* na) -> int32_t {
+    CK_CUDA(cudaMemcpyAsync(h_cnt, a.cnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK_CUDA(cudaStreamSynchronize(st));
+    *na = h_cnt[0];
+    return CK_OK;
+  };
+  int32_t rc;
+  unsigned long long rhs_evals = 0, jac_evals = 0;
+  double slots_act = 0, slots_tot = 0;   // lane utilisation: active slots / lanes issued, summed over the launches
+  const int jblock = jac_tpr_block(m->dev), G = rr_use_warp(m) ? 32 * ((N + 31) / 32) : rr_group(N);
+  auto count_tpr = [&](long long na, int block) { slots_act += (double)na; slots_tot += (double)((na + block - 1) / block) * block; };
+  ros_init_kernel<<<gn, tb, 0, st>>>(a);
+  ros_gather_kernel<<<gn, tb, 0, st>>>(a, N);
+  long long na = n;
+  if (!(o->h0 > 0.0)) {  // EstimateH0: two evaluations
+    if ((rc = ck_rhs(m, na, a.Yw, a.cap, a.Pw, a.F0, a.cap, st))) return fail(rc);
+    ros_h0a_kernel<<<gn, tb, 0, st>>>(a, N);
+    if ((rc = ck_rhs(m, na, a.YT, a.cap, a.Pw, a.FT, a.cap, st))) return fail(rc);
+    ros_h0b_kernel<<<gn, tb, 0, st>>>(a, N);
+    rhs_evals += 2 * (unsigned long long)na;
+  }
+  ros_guard_kernel<<<gn, tb, 0, st>>>(a);
+  ros_swap_kernel<<<1, 1, 0, st>>>(a);
+  std::swap(a.act, a.act2);
+  if ((rc = read_count(&na))) return fail(rc);
+  // the tail (few survivors: a round costs one thread-per-reactor wave whatever the count) goes to the fused kernel
+  const char* te = getenv("CK_ROS_TAIL");
+  const long long tail = te ? atoll(te) : std::min<long long>(2048, std::max<long long>(n / 8, 1));
+  int rounds = 0;
+  while (na >= tail && na > 0) {
+    const unsigned ga = (unsigned)((na + tb - 1) / tb);
+    ros_gather_kernel<<<ga, tb, 0, st>>>(a, N);
+    rc = (jblock == 512) ? launch_jac_rows_rm<512>(m, a, na, sms, st) : launch_jac_rows_rm<224>(m, a, na, sms, st);
+    if (rc) return fail(rc);
+    if ((rc = coop_dispatch(m, a, na, sms, 0, st))) return fail(rc);
+    if ((rc = ck_rhs(m, na, a.YT, a.cap, a.Pw, a.FT, a.cap, st))) return fail(rc);
+    if ((rc = coop_dispatch(m, a, na, sms, 1, st))) return fail(rc);
+    if ((rc = ck_rhs(m, na, a.YT, a.cap, a.Pw, a.FT, a.cap, st))) return fail(rc);
+    if ((rc = coop_dispatch(m, a, na, sms, 2, st))) return fail(rc);
+    ros_swap_kernel<<<1, 1, 0, st>>>(a);
+    std::swap(a.act, a.act2);
+    rhs_evals += 3 * (unsigned long long)na; jac_evals += (unsigned long long)na;
+    count_tpr(na, jblock); count_tpr(na, 512); count_tpr(na, 512);
+    slots_act += 3.0 * na * N; slots_tot += 3.0 * na * G;
+    rounds++;
+    if ((rc = read_count(&na))) return fail(rc);
+  }
+  CK_CUDA(cudaGetLastError());
+  // counters of the rounds (the fused kernel adds its own below)
+  unsigned long long add[2] = {rhs_evals, jac_evals};
+  DevStats* ds = a.stats;
+  CK_CUDA(cudaMemcpyAsync(h_cnt, a.cnt, sizeof(int), cudaMemcpyDeviceToHost, st));   // keep ordering simple
+  CK_CUDA(cudaStreamSynchronize(st));
+  {
+    DevStats hs;
+    CK_CUDA(cudaMemcpy(&hs, ds, sizeof hs, cudaMemcpyDeviceToHost));
+    hs.rhs_evals += add[0]; hs.jac_evals += add[1];
+    hs.lane_active = (unsigned long long)slots_act; hs.lane_total = (unsigned long long)slots_tot;
+    hs.queue = 0;
+    CK_CUDA(cudaMemcpy(ds, &hs, sizeof hs, cudaMemcpyHostToDevice));
+  }
+  if (na > 0) {
+    RosArgs f{};
+    f.n = n; f.ld = ld; f.y = y; f.p = p; f.dt = dt; f.rtol = o->rtol; f.atol = o->atol; f.h0 = o->h0;
+    f.jac_mode = CK_JAC_ANALYTIC; f.max_steps = a.max_steps; f.use_queue = 1;
+    f.n_accept = n_accept; f.n_reject = n_reject; f.status = status; f.h_last = h_last;
+    f.att = a.att; f.stats = a.stats;
+    f.list = a.act; f.list_n = a.cnt; f.rt = a.t; f.rh = a.h; f.rfac = a.fac; f.racc = a.nacc; f.rrej = a.nrej;
+    if ((rc = ros_fused_launch(m, f, na, nullptr, st))) return fail(rc);
+    rounds++;
+  }
+  cudaFreeHost(h_cnt);
+  *rounds_out = rounds;
+  *lane_util = slots_tot > 0 ? slots_act / slots_tot : 1.0;
+  return CK_OK;
+}
+
+}  // namespace ck
+
+// ---- ck_jac_batched: the thread-per-reactor analytic Jacobian through the C ABI ---------------------------------------
+// workspace: f [N][n], HC [2K+1][n], G2 [g2rows][n]
+size_t ck_jac_workspace(const ck_mech* m, int64_t n) {
+  if (n <= 0) return 256;
+  const size_t N = m->K + 1;
+  return al256(N * (size_t)n * 8) + al256((size_t)jac_hc_rows(m->K) * n * 8) + al256((size_t)jac_g2_rows(m->R, m->dev.r_tb) * n * 8);
+}
+
+namespace {
+template <int BLOCK>
+int32_t launch_jac_rows_cm(const ck_mech* m, long long n, const double* y, long long ld, const double* p, const JacOut& o,
+                           cudaStream_t st) {
+  const size_t smem = jac_tpr_smem_bytes(m->K, m->R, m->dev.n_tent, m->dev.rstride, BLOCK);
+  CK_CUDA(cudaFuncSetAttribute(jac_rows_kernel<BLOCK, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int sms = 0;
+  CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  const long long grid = std::max<long long>(1, std::min<long long>((n + BLOCK - 1) / BLOCK, sms));
+  jac_rows_kernel<BLOCK, false><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, n, nullptr, y, ld, p, o);
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}
+}  // namespace
+
+extern "C" int32_t ck_jac_batched(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* J,
+                                  int64_t ldJ, void* ws, size_t ws_bytes, void* stream) {
+  if (!m) { set_error("ck_jac_batched: null mechanism"); return CK_EINVAL; }
+  if (n < 0 || ld < n || ldJ < n) { set_error("ck_jac_batched: bad n/ld"); return CK_EINVAL; }
+  if (n == 0) return CK_OK;
+  if (!y || !p || !J) { set_error("ck_jac_batched: null batch pointer"); return CK_EINVAL; }
+  const int block = jac_tpr_block(m->dev);
+  if (block == 0 || m->dev.rstride > 64) { set_error("ck_jac_batched: %d species do not fit the thread-per-reactor kernel (use ck_jac)", m->K); return CK_EUNSUPPORTED; }
+  if (!ws || ws_bytes < ck_jac_workspace(m, n)) { set_error("ck_jac_batched: workspace of %zu bytes needed", ck_jac_workspace(m, n)); return CK_EWORKSPACE; }
+  CK_CUDA(cudaSetDevice(m->device));
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t N = m->K + 1;
+  char* w = (char*)ws;
+  JacOut o;
+  o.f = (double*)w; o.ldf = n; w += al256(N * (size_t)n * 8);
+  o.hc = (double*)w; o.ldh = n; w += al256((size_t)jac_hc_rows(m->K) * n * 8);
+  o.g2 = (double*)w; o.ldg = n;
+  o.J = J; o.ldJ = ldJ;
+  int32_t rc = (block == 512) ? launch_jac_rows_cm<512>(m, n, y, ld, p, o, st) : launch_jac_rows_cm<224>(m, n, y, ld, p, o, st);
+  if (rc) return rc;
+  jac_trow_kernel<<<(unsigned)((n + 127) / 128), 128, 0, st>>>(m->K, n, o.f, o.ldf, o.hc, o.ldh, J, ldJ);
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}

@@ -112,6 +112,19 @@ def test_ros_c5_subset(oracle):
     _check(g, res, ref, 111)
 
 
+@pytest.mark.parametrize("name,n,ns", [("C3", 777, 53), ("C5", 200, 111), ("C1", 600, 9)])
+def test_ros_batched_rounds_driver(oracle, name, n, ns):
+    """flags bit 3 forces the batched rounds (default only for >= 16384 reactors): same bounds, and the report's counters
+    (3 evaluations + 1 Jacobian per attempt, 2 for EstimateH0) must add up across the rounds and the fused tail."""
+    g, res, ref, mech = _run(oracle, name, n, flags=8)
+    rep = _check(g, res, ref, ns)
+    assert rep["rhs_evals"] == 3 * rep["attempts"] + 2 * n and rep["jac_evals"] == rep["attempts"]
+    assert rep["rounds"] >= 3 and 0 < rep["simt_efficiency"] <= 1
+    g2, res2, _, _ = _run(oracle, name, n, flags=4)          # the fused kernel on the same batch
+    _check(g2, res2, ref, ns)
+    assert res2["report"]["rounds"] == 1
+
+
 def test_ros_static_mapping_gives_same_answer(oracle):
     g, res, ref, mech = _run(oracle, "C1", 300, flags=1)
     _check(g, res, ref, 9)

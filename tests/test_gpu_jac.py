@@ -58,3 +58,20 @@ def test_jac_empty_and_bad_mode():
     y = torch.ones((10, 4), dtype=torch.float64, device="cuda")
     with pytest.raises(ck.CkError):
         M.jac(y, torch.ones(4, dtype=torch.float64, device="cuda"), mode=7)
+
+
+@pytest.mark.parametrize("name,n,nchk", [("C3", 2048 + 77, 10), ("C5", 600, 4), ("C1", 1500, 10)])
+def test_jac_batched_thread_per_reactor_matches_complex_step(oracle, name, n, nchk):
+    """ck_jac_batched (one reactor per lane, one matrix row at a time in tensor memory; row 0 from the species rows
+    through the differentiated enthalpy identity) against the oracle's complex-step Jacobian, and against ck_jac."""
+    M, mech, y, p, torch = _setup(name, n)
+    O = oracle.Mech(mech)
+    yd, pd = torch.from_numpy(y).cuda(), torch.from_numpy(p).cuda()
+    J = M.jac_batched(yd, pd).cpu().numpy()
+    assert np.isfinite(J).all()
+    for r in np.unique(np.concatenate([np.linspace(0, n - 1, nchk).astype(int), [n - 1, n - 2]])):
+        Jc = O.jac(y[:, r], p[r], mode=0)
+        _, Jm = O.jac(y[:, r], p[r], mode=2)
+        err = np.abs(J[:, :, r] - Jc)
+        assert np.all(err <= 1e-12 * Jm + 1e-300), (int(r), float((err / (Jm + 1e-300)).max()),
+                                                     np.unravel_index(np.argmax(err / (Jm + 1e-300)), err.shape))

@@ -39,7 +39,8 @@ def _check(oracle, name, n, ld_pad=0):
     return np.median(rel), rel.max()
 
 
-@pytest.mark.parametrize("name,n", [("C1", 1024), ("C1", 1), ("C1", 129), ("C2", 4096 + 37), ("C5", 300)])
+@pytest.mark.parametrize("name,n", [("C1", 1024), ("C1", 1), ("C1", 129), ("C2", 1000), ("C2", 4096 + 37), ("C5", 300),
+                                    ("C5", 4096 + 19), ("C1", 2048 + 5)])
 def test_rhs_matches_oracle(oracle, name, n):
     med, mx = _check(oracle, name, n)
     assert med < 1e-13

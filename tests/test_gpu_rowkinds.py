@@ -74,10 +74,23 @@ def test_jac_both_modes(oracle, name, n, nchk):
         assert np.all((np.abs(Jf[:, :, r] - Jo) <= 1e-5 * colscale)[:, major])
 
 
-def _integrate_check(oracle, name, n, solver, dt, jac_mode=0):
+@pytest.mark.parametrize("name,n,nchk", [("rk14", 700, 6), ("rk20", 700, 6), ("h2co", 700, 5), ("c1irr", 600, 4)])
+def test_jac_batched(oracle, name, n, nchk):
+    M, mech, y, p, torch = _setup(name, n)
+    O = oracle.Mech(mech)
+    J = M.jac_batched(torch.from_numpy(y).cuda(), torch.from_numpy(p).cuda()).cpu().numpy()
+    assert np.isfinite(J).all()
+    for r in np.linspace(0, n - 1, nchk).astype(int):
+        Jc = O.jac(y[:, r], p[r], mode=0)
+        _, Jm = O.jac(y[:, r], p[r], mode=2)
+        err = np.abs(J[:, :, r] - Jc)
+        assert np.all(err <= 1e-12 * Jm + 1e-300), (int(r), float((err / (Jm + 1e-300)).max()))
+
+
+def _integrate_check(oracle, name, n, solver, dt, jac_mode=0, flags=0):
     M, mech, y, p, torch = _setup(name, n)
     yd = torch.from_numpy(y).cuda()
-    res = M.integrate(solver, yd, torch.from_numpy(p).cuda(), dt, jac_mode=jac_mode)
+    res = M.integrate(solver, yd, torch.from_numpy(p).cuda(), dt, jac_mode=jac_mode, flags=flags)
     torch.cuda.synchronize()
     g = yd.cpu().numpy()
     ref = oracle.Mech(mech).integrate(solver, y, p, dt, jac_mode=jac_mode, nthreads=16)
@@ -117,6 +130,13 @@ def _integrate_check(oracle, name, n, solver, dt, jac_mode=0):
                                        ("rk130", 24, 1e-6)])
 def test_ros_analytic(oracle, name, n, dt):
     _integrate_check(oracle, name, n, "ros", dt)
+
+
+@pytest.mark.parametrize("name,n,dt", [("rk14", 600, 5e-6), ("rk20", 600, 2e-5), ("h2co", 600, 1e-5), ("c1irr", 400, 1e-6)])
+def test_ros_batched_rounds(oracle, name, n, dt):
+    """flags bit 3: the batched-rounds driver (thread-per-reactor chemistry, cooperative LU) on small batches."""
+    rep = _integrate_check(oracle, name, n, "ros", dt, flags=8)
+    assert rep["rounds"] >= 2
 
 
 @pytest.mark.parametrize("name,n,dt", [("rk14", 150, 5e-6), ("rk20", 150, 2e-5), ("c1irr", 64, 1e-6), ("rk130", 8, 1e-6)])
