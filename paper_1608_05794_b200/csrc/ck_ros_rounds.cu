@@ -759,7 +759,7 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   if ((rc = read_count(&na))) return fail(rc);
   // the tail (few survivors: a round costs one thread-per-reactor wave whatever the count) goes to the fused kernel
   const char* te = getenv("CK_ROS_TAIL");
-  const long long tail = te ? atoll(te) : std::min<long long>(2048, std::max<long long>(n / 8, 1));
+  const long long tail = te ? atoll(te) : std::min<long long>(4096, std::max<long long>(n / 8, 1));
   int rounds = 0;
   while (na >= tail && na > 0) {
     const unsigned ga = (unsigned)((na + tb - 1) / tb);

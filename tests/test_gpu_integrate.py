@@ -44,7 +44,8 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
     """fd: ROS4 with the finite-difference Jacobian.  Its columns carry rounding noise eps D / sigma_j (reading G12), which
     differs between any two correct executions and which the step controller amplifies: the two CPU builds of the oracle
     already differ by 2 accepted / 6 rejected attempts per reactor (tests/test_oracle_p3.py), so the count slack is 2
-    instead of 1, the batch total of rejected attempts may differ by 10 %, and states are judged by DESIGN.md P3."""
+    (6 for rejected attempts) instead of 1, the batch total of rejected attempts may differ by 10 %, and states are
+    judged by DESIGN.md P3."""
     slack = 2 if fd else 1
     st = res["status"].cpu().numpy()
     assert np.array_equal(st, ref["status"]) and np.all(st == 0)
@@ -73,7 +74,7 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
     assert abs(int(nr.sum()) - int(ref["n_reject"].sum())) <= max((2 if fd else 1) * frac_count * ref["n_reject"].sum(), 1), (int(nr.sum()), int(ref["n_reject"].sum()))
     d = np.abs(nr - ref["n_reject"])
     print("n_reject |d| max", int(d.max()), "mean", float(d.mean()), "ref mean", float(ref["n_reject"].mean()))
-    assert np.all(d <= np.maximum(slack, np.ceil(frac_count * att_ref))), int(d.max())
+    assert np.all(d <= np.maximum(6 if fd else 1, np.ceil(frac_count * att_ref))), int(d.max())
     rep = res["report"]
     assert rep["accepted"] == int(na.sum()) and rep["rejected"] == int(nr.sum())
     assert rep["attempts"] == rep["accepted"] + rep["rejected"] and rep["n_failed"] == 0

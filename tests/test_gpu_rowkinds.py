@@ -113,10 +113,12 @@ def _integrate_check(oracle, name, n, solver, dt, jac_mode=0, flags=0):
             e_cpu = np.sqrt(np.mean(((ref["y"][:, r] - col) / sc) ** 2))
             assert e_gpu <= 2.0 * e_cpu + 1.0, (int(r), float(e_gpu), float(e_cpu))
     att = ref["n_accept"] + ref["n_reject"]
-    slack = 2 if jac_mode else 1
+    # FD Jacobian: the two CPU builds of the oracle already differ by 2 accepted / 6 rejected attempts per reactor
+    # (tests/test_oracle_p3.py), so that is the slack granted here; analytic Jacobian: 1
+    slack = {"n_accept": 2 if jac_mode else 1, "n_reject": 6 if jac_mode else 1}
     for key in ("n_accept", "n_reject"):                    # DESIGN.md P2, applied to rejected attempts too
         a, b = res[key].cpu().numpy(), ref[key]
-        lim = np.maximum(slack, np.ceil(0.05 * (b if key == "n_accept" else att)))
+        lim = np.maximum(slack[key], np.ceil(0.05 * (b if key == "n_accept" else att)))
         assert np.all(np.abs(a - b) <= lim), (key, int(np.abs(a - b).max()))
     rep = res["report"]
     N = mech["n_species"] + 1

@@ -61,7 +61,7 @@ def test_fd_jacobian_makes_step_counts_depend_on_the_last_bit(oracle):
     """ROS4: with the complex-step Jacobian the two CPU builds take identical accept / reject decisions; with the
     finite-difference Jacobian (increment of reading G12) the rounding noise eps D / sigma_j of its columns
     differs between them and so do the step counts -- the slack tests/test_gpu_integrate.py grants FD runs (2 instead of
-    1 attempt per reactor) is what two CPU executions already need."""
+    1 accepted, 6 instead of 1 rejected attempts per reactor) is what two CPU executions already need."""
     mech, y, p, cfg = make_config("C1", n=200)
     A = oracle.Mech(mech)
     B = oracle.Mech(mech, variant="fma")
@@ -73,4 +73,4 @@ def test_fd_jacobian_makes_step_counts_depend_on_the_last_bit(oracle):
                    (np.abs(ra["y"] - rb["y"]) / np.maximum(np.abs(ra["y"]), 1e-5)).max())
     assert out[0][0] == 0 and out[0][1] == 0 and out[0][2] < 1e-11
     assert out[1][0] >= 1 and out[1][1] >= 2 and out[1][2] > 1e-8
-    assert out[1][0] <= 2 and out[1][2] < 1e-5
+    assert out[1][0] <= 2 and out[1][1] <= 6 and out[1][2] < 1e-5    # the slack the GPU tests grant FD runs
