@@ -24,6 +24,23 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
   return s;
 }
 
+// two sums with one barrier pair; red: >= 2 * (G / 32) doubles
+template <int G>
+__device__ __forceinline__ void block_sum2(double& a, double& b, double* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
+  if (G == 32) return;
+  constexpr int W = G / 32;
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  __syncthreads();
+  if (l == 0) { red[w] = a; red[W + w] = b; }
+  __syncthreads();
+  double sa = 0.0, sb = 0.0;
+#pragma unroll
+  for (int i = 0; i < W; ++i) { sa += red[i]; sb += red[W + i]; }
+  a = sa; b = sb;
+}
+
 // Shared-memory working set of the cooperative chemistry (pointers into the CTA's dynamic smem)
 struct CoopChem {
   double* C;     // [K+1] concentrations, C[K] = 1
@@ -43,6 +60,8 @@ struct CoopChem {
   double* tau;   // [K]    sum_i nu_ki dq_i/dT|_C
   int* dsl;      // [6][R] slot species of every reaction (shared-memory copy: the row assembly would otherwise
                  //        wait on a global load per reaction)
+  const int* tptr;  // transposed stoichiometry for the production-rate gather of rhs_wide: shared-memory copies when
+  const int* tent;  //        the caller staged them (rkf45_coop_kernel), else the global arrays
 };
 struct CoopScalars { double rho, S, cps, Ctot, hw; };
 
@@ -69,6 +88,7 @@ __device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool 
   c.sig = base; base += jac ? K : 0;
   c.tau = base; base += jac ? K : 0;
   c.dsl = reinterpret_cast<int*>(base);
+  c.tptr = nullptr; c.tent = nullptr;
   return c;
 }
 
@@ -146,6 +166,92 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
   if (tid == 0) fout[0] = -(t.T * s.hw) / (s.rho * s.cps);
   __syncthreads();
   return s;
+}
+
+// f = RHS(y; p) with a WIDE CTA (G >= 4 warps, ideally G >= R): the latency-optimised evaluation for the serial step
+// chains of the RKF45 stragglers (ck_rkf.cu).  One thread per species for the thermo, one thread per reaction for the
+// rates of progress (a single trip when G >= R), QS adjacent lanes per species for the production-rate gather.  Nothing
+// is computed redundantly: the logarithm of T is taken by one thread, the reductions run only in the warps that hold
+// data, and every thread picks the few partial sums up after a barrier (five barriers per evaluation).  Constants come
+// through L1 (this kernel leaves it almost all of the SM's 228 KB).  Ends with a __syncthreads().
+template <int G>
+__device__ __forceinline__ void rhs_wide(const MechDev& m, const double* __restrict__ y, double p, double* __restrict__ fout,
+                                         const CoopChem& c, TState& t) {
+  const int K = m.K, R = m.R, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int KW = (K + 31) >> 5;          // warps holding species in the thermo phase
+  const double T = y[0];
+  double yw = 0.0, cp = 0.0;
+  if (warp == KW && lane == 0) {         // a warp without species: T-state for everybody
+    const TState ts = make_tstate(m, T);
+    c.red[32] = ts.lnT; c.red[33] = ts.invT; c.red[34] = (double)ts.tint;
+  }
+  if (warp < KW) {
+    if (tid < K) {
+      TState tt;
+      tt.T = T; tt.invT = 1.0 / T; tt.lnT = 0.0; tt.tint = 0;
+      double cpR, hRT;
+      thermo_cp_h(m, tid, tt, cpR, hRT);
+      yw = y[1 + tid] * __ldg(m.invW + tid);
+      c.hRT[tid] = hRT;
+      cp = yw * cpR;
+    }
+    double S = yw;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { S += __shfl_xor_sync(0xffffffffu, S, o); cp += __shfl_xor_sync(0xffffffffu, cp, o); }
+    if (lane == 0) { c.red[warp] = S; c.red[8 + warp] = cp; }
+  }
+  __syncthreads();
+  double S = 0.0, cps = 0.0;
+  for (int w = 0; w < KW; ++w) { S += c.red[w]; cps += c.red[8 + w]; }
+  t.T = T; t.lnT = c.red[32]; t.invT = c.red[33]; t.tint = (int)c.red[34];
+  const double Ctot = p * t.invT * (1.0 / R_U), rho = Ctot / S;
+  if (tid < K) c.C[tid] = rho * yw;
+  if (tid == 0) c.C[K] = 1.0;
+  __syncthreads();
+  for (int r = tid; r < R; r += G) {
+    const RxnConst kc = load_rxn_global(m, r, t.tint);
+    c.q[r] = reaction_q<1, false>(m, r, kc, t, c.C, Ctot, nullptr);
+  }
+  __syncthreads();
+  // QS adjacent lanes share one species row of the transposed stoichiometry
+  const int QS = (4 * K <= G) ? 4 : ((2 * K <= G) ? 2 : 1);
+  const int GW = (K * QS + 31) >> 5;     // warps holding species in the gather phase
+  const double irho = 1.0 / rho;
+  if (warp < GW) {
+    const int k = tid / QS, part = tid % QS;
+    const int* tptr = c.tptr ? c.tptr : m.tptr;
+    const int* tent = c.tent ? c.tent : m.tent;
+    double w = 0.0;
+    if (k < K) {
+      int e = tptr[k] + part;
+      const int e1 = tptr[k + 1];
+      double w1 = 0.0;
+      for (; e + QS < e1; e += 2 * QS) {   // two independent chains
+        const int en0 = tent[e], en1 = tent[e + QS];
+        w = fma((double)((en0 & 255) - 128), c.q[en0 >> 8], w);
+        w1 = fma((double)((en1 & 255) - 128), c.q[en1 >> 8], w1);
+      }
+      if (e < e1) { const int en0 = tent[e]; w = fma((double)((en0 & 255) - 128), c.q[en0 >> 8], w); }
+      w += w1;
+    }
+    if (QS >= 2) w += __shfl_xor_sync(0xffffffffu, w, 1);
+    if (QS >= 4) w += __shfl_xor_sync(0xffffffffu, w, 2);
+    double hwp = 0.0;
+    if (k < K && part == 0) {
+      hwp = c.hRT[k] * w;
+      fout[1 + k] = w * __ldg(m.W + k) * irho;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) hwp += __shfl_xor_sync(0xffffffffu, hwp, o);
+    if (lane == 0) c.red[16 + warp] = hwp;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double hw = 0.0;
+    for (int w = 0; w < GW; ++w) hw += c.red[16 + w];
+    fout[0] = -(t.T * hw) / (rho * cps);
+  }
+  __syncthreads();
 }
 
 // f(y) AND the species rows G_kj of the analytic Jacobian in one pass over the reactions, G reactions at a time:

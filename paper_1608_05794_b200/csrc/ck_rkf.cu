@@ -50,6 +50,7 @@ struct RkfArgs {
   int* rec_acc;         // [n]
   int* rec_rej;         // [n]
   int evict;            // 1: end-game eviction enabled
+  double big_steps;     // predicted remaining attempts above which an evicted reactor counts as a straggler
   double* V;  // [8][N][nslots]: 0 = y_n, 1..6 = f evaluations, 7 = stage argument
   DevStats* stats;
 };
@@ -101,7 +102,10 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
     if (endgame) {  // re-batch: hand this reactor to the cooperative finisher (state is at an attempt boundary)
       for (int c = 0; c < N; ++c) a.y[(size_t)c * a.ld + r] = Vy[c * ns];
       a.rec_t[r] = t; a.rec_h[r] = h; a.rec_fac[r] = fac_max; a.rec_acc[r] = nacc; a.rec_rej[r] = nrej;
-      a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
+      // two classes: reactors whose predicted number of remaining attempts (t_f - t) / h is large go to the wide,
+      // latency-optimised finisher (one CTA per SM each), the mass to the throughput-oriented one
+      if ((a.dt - t) > a.big_steps * h) a.elist[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_b, 1ULL)] = (int)r;
+      else a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
       r = -1;
       return true;
     }
@@ -248,25 +252,36 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
 // stragglers of the step-count distribution) are completed CTA-per-reactor, so that one
 // reactor's long serial chain of attempts runs at the latency of a cooperative RHS (G lanes share one
 // evaluation) instead of holding a mostly idle CTA of the throughput kernel.
-__host__ __device__ inline size_t rkf_coop_smem_doubles(int K, int R) { return (size_t)8 * (K + 1) + coop_chem_doubles(K, R, false); }
+__host__ __device__ inline size_t rkf_coop_smem_doubles(int K, int R, int n_tent) {
+  return (size_t)8 * (K + 1) + coop_chem_doubles(K, R, false) + (size_t)((n_tent + K + 2 + 1) >> 1);
+}
 
-template <int G>
-__global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const RkfArgs a) {
+// WIDE: the latency-optimised evaluation rhs_wide (G = 384 threads, one reaction per thread for R <= 384)
+template <int G, bool WIDE>
+__global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const RkfArgs a, const int cls) {
   extern __shared__ double sm[];
   __shared__ long long s_next;
   const int N = m.K + 1, tid = threadIdx.x;
   double* Y = sm;            // y_n
   double* F = sm + N;        // six evaluation vectors F[j*N + c]
   double* YT = sm + 7 * N;   // stage argument / candidate
-  const CoopChem c = coop_carve(sm + 8 * N, m.K, m.R, false);
-  const long long n_ev = (long long)a.stats->n_evicted;
+  CoopChem c = coop_carve(sm + 8 * N, m.K, m.R, false);
+  if (WIDE) {  // the gather lists of rhs_wide, staged once per CTA
+    int* s_tptr = reinterpret_cast<int*>(sm + 8 * N + coop_chem_doubles(m.K, m.R, false));
+    int* s_tent = s_tptr + m.K + 1;
+    for (int i = tid; i <= m.K; i += G) s_tptr[i] = __ldg(m.tptr + i);
+    for (int i = tid; i < m.n_tent; i += G) s_tent[i] = __ldg(m.tent + i);
+    c.tptr = s_tptr; c.tent = s_tent;
+    __syncthreads();
+  }
+  const long long n_ev = (long long)(cls ? a.stats->n_evicted_b : a.stats->n_evicted);
   unsigned long long c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
   for (;;) {
     __syncthreads();
-    if (tid == 0) s_next = (long long)atomicAdd(&a.stats->queue2, 1ULL);
+    if (tid == 0) s_next = (long long)atomicAdd(cls ? &a.stats->queue_b : &a.stats->queue2, 1ULL);
     __syncthreads();
     if (s_next >= n_ev) break;
-    const long long r = a.elist[s_next];
+    const long long r = a.elist[cls ? a.n - 1 - s_next : s_next];
     const double p = a.p[r];
     for (int i = tid; i < N; i += G) Y[i] = a.y[(size_t)i * a.ld + r];
     double t = a.rec_t[r], h = a.rec_h[r], fac_max = a.rec_fac[r], h_used = 0.0;
@@ -279,7 +294,8 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
       bool last = false;
       if (h >= a.dt - t) { h = a.dt - t; last = true; }
       TState ts;
-      rhs_coop<G, false>(m, Y, p, F, c, ts);
+      if constexpr (WIDE) rhs_wide<G>(m, Y, p, F, c, ts);
+      else rhs_coop<G, false>(m, Y, p, F, c, ts);
       for (int s = 0; s < 5; ++s) {
         for (int i = tid; i < N; i += G) {
           double acc = 0.0;
@@ -287,7 +303,8 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
           YT[i] = fma(h, acc, Y[i]);
         }
         __syncthreads();
-        rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
+        if constexpr (WIDE) rhs_wide<G>(m, YT, p, F + (s + 1) * N, c, ts);
+        else rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
       }
       c_rhs += 6;
       double es = 0.0;
@@ -422,6 +439,7 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   a.rec_fac = (double*)wp; wp += bd;
   a.V = (double*)wp;
   a.evict = (o->flags & 3) ? 0 : 1;  // bit 0: static mapping, bit 1: refill only (no finisher)
+  a.big_steps = (m->K + 1 > 32) ? 2000.0 : 1e300;
   switch (pl.block) {
     case 512: rkf45_kernel<512, true><<<(unsigned)pl.grid, 512, pl.smem, st>>>(m->dev, a); break;
     case 256: rkf45_kernel<256, false><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
@@ -432,7 +450,7 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   CK_CUDA(cudaGetLastError());
   int rounds = 1;
   if (a.evict) {  // finisher over the eviction list (its length is read on the device)
-    const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R) * sizeof(double);
+    const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R, m->dev.n_tent) * sizeof(double);
     if (smem2 > 227 * 1024) { set_error("ck_integrate_rkf45: mechanism too large for the cooperative finisher"); return CK_EUNSUPPORTED; }
     int per_sm = 0, sms = 0;
     const int N = m->K + 1;
@@ -440,19 +458,21 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
     // threads per evicted reactor: the finisher runs the stragglers' serial chains, so its time is the latency of one
     // cooperative RHS x 6 x the attempts of the slowest reactor; wider CTAs shorten the reaction loop of that RHS
     const long long cap = (long long)n;
-    auto launch_fin = [&](auto kern, int G) -> int32_t {
+    auto launch_fin = [&](auto kern, int G, int cls) -> int32_t {
       CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
       CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G, smem2));
-      kern<<<(unsigned)std::min<long long>(cap, (long long)std::max(per_sm, 1) * sms), G, smem2, st>>>(m->dev, a);
+      kern<<<(unsigned)std::min<long long>(cap, (long long)std::max(per_sm, 1) * sms), G, smem2, st>>>(m->dev, a, cls);
       return CK_OK;
     };
+    // the mass of the evicted reactors: many narrow CTAs per SM (throughput); the predicted stragglers: one wide CTA each
     int32_t rcf;
-    if (N <= 32) rcf = launch_fin(rkf45_coop_kernel<32>, 32);
-    else if (N <= 64) rcf = launch_fin(rkf45_coop_kernel<64>, 64);
-    else rcf = launch_fin(rkf45_coop_kernel<128>, 128);
+    if (N <= 32) rcf = launch_fin(rkf45_coop_kernel<32, false>, 32, 0);
+    else if (N <= 64) rcf = launch_fin(rkf45_coop_kernel<64, false>, 64, 0);
+    else rcf = launch_fin(rkf45_coop_kernel<128, false>, 128, 0);
     if (rcf) return rcf;
+    if (N > 32) { rcf = launch_fin(rkf45_coop_kernel<384, true>, 384, 1); if (rcf) return rcf; }
     CK_CUDA(cudaGetLastError());
-    rounds = 2;
+    rounds = (N > 32) ? 3 : 2;
   }
   return integrate_report(m, n, a.att, a.stats, rounds, 0, report, st);
 }

@@ -17,7 +17,10 @@ struct DevStats {
   unsigned long long qempty;       // set once the main queue ran dry
   unsigned long long clk[8];       // ROS4 phase clocks (SM cycles summed over CTAs): 0 RHS+dq, 1 Jacobian assembly,
                                    // 2 LU, 3 solves, 4 stage RHS, 5 vectors/control, 6 total
-  unsigned long long pad[12];
+  unsigned long long n_evicted_b;  // ... of which predicted stragglers (handed to the wide low-latency finisher; listed from
+                                   // the back of the eviction list)
+  unsigned long long queue_b;      // work-queue head of the wide finisher
+  unsigned long long pad[10];
 };
 static_assert(sizeof(DevStats) == 256, "DevStats is the 256-byte header of the workspace");
 
