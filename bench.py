@@ -30,7 +30,17 @@ UNIT = "RHS evals/s"
 # FP64 vector peak derived from unit counts and clocks:
 # 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
 PEAK_SLOTS = 148 * 64 * 1.965e9
-RHS_DRAM_BYTES_PER_STATE = 690.0  # measured (profiles/r01_rhs_kernel_full.md); algorithmic: (2K+3)*8 = 872 B
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE rhs_kernel_tmem<512> launch over the full 1,048,576 states
+# (ncu --set full, profiles/r02_rhs_kernel_full.md); None until such a capture of the full-size launch exists
+RHS_DRAM_BYTES_PER_LAUNCH_FULL = 865.98e6
+
+
+def measured_hbm_gbs():
+    """HBM copy bandwidth the driver measured on this pool (MEASURED_PEAKS.json); fallback of the profiling guide."""
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
 
 
 class ClockSampler:
@@ -150,12 +160,30 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def integrator_extras(torch, ck, dev):
-    """Reactors/s of the integrators on configs 3-5 (device-resident inputs), best of 2 after one warm-up.
-    Returns {} entries with an "error" key while an integrator is not available."""
+def time_oracle_integrate(mech, y, p, cfg, n_sub):
+    """Oracle integrator (as it stands) on the first n_sub reactors of the workload, all host cores (omp dynamic over
+    reactors, the structure of the paper's own baseline)."""
+    from oracle import ck_oracle
+    O = ck_oracle.Mech(mech)
+    cores = min(oracle_cores(), ck_oracle.max_threads())
+    ys = np.ascontiguousarray(y[:, :n_sub]); ps = np.ascontiguousarray(p[:n_sub])
+    t0 = time.perf_counter()
+    r = O.integrate(cfg["call"], ys, ps, cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"], nthreads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": n_sub / dt, "unit": "reactors/s", "rhs_evals_per_s": r["rhs_evals"] / dt, "cores": cores, "kind": "oracle",
+            "sample": f"first {n_sub} reactors of the workload, {dt:.1f} s, omp dynamic over reactors"}
+
+
+# reactors the oracle integrates for the CPU baseline of each integration config (a few seconds each on 16 cores)
+ORACLE_SUBSET = {"C1": 1024, "C3": 2048, "C4": 2048, "C5": 512, "C6": 4096, "C7": 2048}
+
+
+def integrator_extras(torch, ck, dev, cpu=True):
+    """Reactors/s of the integrators on configs 1, 3-7 (device-resident inputs, best of 2 after one warm-up), the same
+    through the host-pointer entry point (transfers inside the call), and the oracle on a subset of the same workload."""
     from synth_inputs import make_config
     out = {}
-    for name in ("C1", "C3", "C4", "C5"):
+    for name in ("C1", "C3", "C4", "C5", "C6", "C7"):
         try:
             mech, y, p, cfg = make_config(name)
             M = ck.Mechanism(mech, device=dev.index or 0)
@@ -174,13 +202,14 @@ def integrator_extras(torch, ck, dev):
                     best = ms if best is None else min(best, ms)
             rep = res["report"]
             slots_rhs = M.rhs_slots()
-            out[name] = {"call": cfg["call"], "n": int(y.shape[1]), "ms": best, "reactors_per_s": y.shape[1] / (best * 1e-3),
+            n = int(y.shape[1])
+            out[name] = {"call": cfg["call"], "n": n, "ms": best, "reactors_per_s": n / (best * 1e-3),
                          "rhs_evals_per_s": rep["rhs_evals"] / (best * 1e-3), "attempts": rep["attempts"],
                          "accepted": rep["accepted"], "rejected": rep["rejected"], "rounds": rep["rounds"],
                          "simt_efficiency": rep["simt_efficiency"], "waste_p32_static": rep["waste_p32"],
                          "n_failed": rep["n_failed"],
                          "rhs_only_roofline_frac": rep["rhs_evals"] * slots_rhs / (best * 1e-3) / PEAK_SLOTS}
-            # algorithmic FP64-pipe instructions of the whole integration (SURVEY.md section 8(d), DESIGN.md section 5):
+            # algorithmic FP64-pipe instructions of the whole integration (SURVEY.md section 8(d), DESIGN.md section 6):
             # every RHS evaluation, an analytic Jacobian at 2.1 RHS, N^3/3 per LU, 4 N^2 per attempt for the four
             # stage solves, ~20 N per attempt for the stage vectors, error norm and step control
             Nn = int(y.shape[0])
@@ -188,22 +217,74 @@ def integrator_extras(torch, ck, dev):
                 + (4.0 * Nn * Nn if cfg["call"] == "ros" else 0.0) * rep["attempts"] + 20.0 * Nn * rep["attempts"]
             out[name]["alg_fp64_inst_per_attempt"] = slots / max(rep["attempts"], 1)
             out[name]["roofline_frac"] = slots / (best * 1e-3) / PEAK_SLOTS
-            # waste study (Eq. 20 and Figs. 9-10): mean and upper decile of
-            # W over the static work units at the paper's four SIMD widths, from this run's step counts (ck_waste)
+            # end to end through ck_integrate_host: pinned host buffers, H2D + integration + D2H of states and step counts
+            yh = torch.from_numpy(y).pin_memory(); ph = torch.from_numpy(p).pin_memory()
+            work = torch.empty_like(yh).pin_memory()
+            tbest = None
+            for it in range(2):
+                work.copy_(yh)
+                torch.cuda.synchronize(); t0 = time.perf_counter()
+                M.integrate_host(cfg["call"], work.numpy(), ph.numpy(), cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"])
+                te = time.perf_counter() - t0
+                if it >= 1 or tbest is None:
+                    tbest = te
+            out[name]["e2e"] = {"value": n / tbest, "unit": "reactors/s", "h2d_bytes_per_step": int(yh.numel() * 8 + ph.numel() * 8),
+                                "d2h_bytes_per_step": int(yh.numel() * 8 + n * 20)}
+            # waste study (Eq. 20 and Figs. 9-10): mean, upper decile and the
+            # CDF point the paper quotes (share of work units with W < 1 %: 92 % at width 4, 63 % at width 32 for its
+            # RKF45 flame data) at the paper's four SIMD widths, from this run's step counts (ck_waste);
+            # and the same with 4 / 16 reactors per lane (several tasks per thread)
             ws_ = {}
             for P in (4, 8, 16, 32):
                 Wd = M.waste(res["n_accept"], res["n_reject"], P)
-                ws_[str(P)] = {"mean": float(Wd.mean()), "p90": float(torch.quantile(Wd, 0.9))}
+                ws_[str(P)] = {"mean": float(Wd.mean()), "p90": float(torch.quantile(Wd, 0.9)),
+                               "frac_units_below_1pct": float((Wd < 0.01).double().mean()),
+                               "frac_units_below_10pct": float((Wd < 0.10).double().mean()),
+                               "mean_4_tasks_per_lane": float(M.waste(res["n_accept"], res["n_reject"], P, tasks=4).mean()),
+                               "mean_16_tasks_per_lane": float(M.waste(res["n_accept"], res["n_reject"], P, tasks=16).mean())}
             out[name]["waste_static"] = ws_
             if name == "C3":  # the same batch in flame order: neighbours need similar step counts
                 _, yf, pf, _ = make_config(name, flame_ordered=True)
                 rf = M.integrate(cfg["call"], torch.from_numpy(yf).to(dev), torch.from_numpy(pf).to(dev), cfg["dt"],
                                  rtol=cfg["rtol"], atol=cfg["atol"], ws=ws)
                 out[name]["waste_static_flame_ordered"] = {
-                    str(P): {"mean": float(M.waste(rf["n_accept"], rf["n_reject"], P).mean())} for P in (4, 8, 16, 32)}
+                    str(P): {"mean": float(M.waste(rf["n_accept"], rf["n_reject"], P).mean()),
+                             "frac_units_below_1pct": float((M.waste(rf["n_accept"], rf["n_reject"], P) < 0.01).double().mean())}
+                    for P in (4, 8, 16, 32)}
+            if cpu:
+                out[name]["cpu_baseline"] = time_oracle_integrate(mech, y, p, cfg, min(ORACLE_SUBSET[name], n))
             M.close()
-        except Exception as ex:  # integrator not available yet / failed: report, do not hide
+        except Exception as ex:  # report, do not hide
             out[name] = {"error": str(ex)[:200]}
+    return out
+
+
+def rhs_extras(torch, ck, dev, steps=10):
+    """RHS-only throughput and roofline fraction on the other model shapes (same state recipe as config 2, 1,048,576
+    states): the 111-species / 784-reaction model (tensor-memory kernel with 224-thread CTAs) and the 14 / 38 model."""
+    from synth_inputs import states as S
+    from synth_inputs.configs import get_mech
+    out = {}
+    for label, mname, n in (("111sp_784rxn", "c4", 1048576), ("14sp_38rxn", "h2co", 1048576), ("53sp_634irrev", "c1irr", 1048576)):
+        try:
+            mech = get_mech(mname)
+            y, p = S.dirichlet_states(mech, n, 108)
+            M = ck.Mechanism(mech, device=dev.index or 0)
+            yd = torch.from_numpy(y).to(dev); pd = torch.from_numpy(p).to(dev); o = torch.empty_like(yd)
+            for _ in range(3):
+                M.rhs(yd, pd, out=o)
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); e0.record()
+            for _ in range(steps):
+                M.rhs(yd, pd, out=o)
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            out[label] = {"n": n, "ms_per_pass": ms, "rhs_evals_per_s": n / (ms * 1e-3), "kernel": M.rhs_kernel_name(n),
+                          "slots_per_eval": M.rhs_slots(), "roofline_frac": M.rhs_slots() * n / (ms * 1e-3) / PEAK_SLOTS}
+            M.close()
+            del yd, o
+        except Exception as ex:
+            out[label] = {"error": str(ex)[:200]}
     return out
 
 
@@ -278,18 +359,20 @@ def run_ours(args):
         measured_peak = ck.fp64_peak(local)
     except Exception:
         pass
-    # dram__bytes_read.sum + dram__bytes_write.sum of ck::rhs_kernel from the ncu --set full capture summarised in
-    # profiles/r01_rhs_kernel_full.md (683 B per state at 262,144 states), scaled to this launch's state count
-    traffic = RHS_DRAM_BYTES_PER_STATE * n
-    roofline = {"bound": "alu", "kernel": "ck::rhs_kernel_tmem<512>", "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
+    traffic = RHS_DRAM_BYTES_PER_LAUNCH_FULL if n == 1048576 else None
+    hbm_gbs, hbm_src = measured_hbm_gbs()
+    roofline = {"bound": "alu", "kernel": M.rhs_kernel_name(n), "achieved": 2 * achieved / 1e12, "peak": 2 * PEAK_SLOTS / 1e12,
                 "unit": "TFLOP/s", "frac": achieved / PEAK_SLOTS, "traffic": traffic,
-                "peak_source": "derived: 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
+                "peak_source": "derived and probed FP64 peak (MEASURED_PEAKS.json carries no FP64 figure): 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
                 "slots_per_eval": slots, "fp64_pipe_inst_per_s": achieved,
                 "measured_dfma_peak_inst_per_s": measured_peak,
                 "frac_of_measured_dfma_peak": (achieved / measured_peak) if measured_peak else None,
                 "hbm_alg_bytes_per_launch": alg_bytes, "hbm_achieved_GBs": alg_bytes / (per_launch_ms * 1e-3) / 1e9,
-                "hbm_frac_of_measured": alg_bytes / (per_launch_ms * 1e-3) / 1e9 / 6554.2}
+                "hbm_peak_GBs": hbm_gbs, "hbm_peak_source": hbm_src,
+                "hbm_frac_of_measured": alg_bytes / (per_launch_ms * 1e-3) / 1e9 / hbm_gbs}
     cpu_v, cores, ns, cpu_dt = time_oracle_rhs(mech, y, p)
+    del yd, out, yh, ph, oh
+    torch.cuda.empty_cache()
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
@@ -301,6 +384,7 @@ def run_ours(args):
                              "sample": f"{ns} state evaluations (passes over the first 262,144 of {n} states), {cpu_dt:.1f} s, omp dynamic over states"}}
     if args.extras:
         line["integrators"] = integrator_extras(torch, ck, dev)
+        line["rhs_other_models"] = rhs_extras(torch, ck, dev)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

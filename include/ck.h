@@ -153,6 +153,9 @@ int32_t ck_integrate_host(ck_mech* m, int32_t op, int64_t n, double* y_inout, in
 /* Roofline support: FP64 instruction count ("slots": DFMA/DMUL/DADD, transcendental at their FP64-pipe
  * instruction counts) that one RHS evaluation of this mechanism needs algorithmically. */
 int32_t ck_rhs_slots(const ck_mech* m, double* slots);
+/* Which kernel ck_rhs launches for n states of this model: threads per CTA and whether the production-rate
+ * accumulators live in tensor memory (rhs_kernel_tmem<block>) or in shared memory (rhs_kernel<block>). */
+int32_t ck_rhs_variant(const ck_mech* m, int64_t n, int32_t* block, int32_t* tmem);
 /* Measure the FP64 FMA peak of the device with a register-resident DFMA chain (slots/s). */
 int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream);
 
@@ -162,6 +165,12 @@ int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream);
  * caller; W has ceil(n / P) entries.  The ragged last unit divides by the lanes it has; a unit whose reactors took
  * no step has W = 0.  P in [1, 1024].  Enqueues on `stream`. */
 int32_t ck_waste(int64_t n, const int32_t* n_accept, const int32_t* n_reject, int32_t P, double* W, void* stream);
+/* The same metric when every lane works through `tasks` reactors instead of one (the mitigation of Murray's ref. [48],
+ * PAPER.md:419): unit j holds P x tasks consecutive reactors, lane l takes reactors l, l + P, l + 2 P, ... of the unit,
+ * its cost is the sum of their attempts, W_j = 1 - sum_i N_i / (lanes x max_l cost_l), lanes = lanes that own at least
+ * one reactor.  W has ceil(n / (P tasks)) entries; tasks = 1 is ck_waste.  1 <= tasks <= 4096. */
+int32_t ck_waste_tasks(int64_t n, const int32_t* n_accept, const int32_t* n_reject, int32_t P, int32_t tasks, double* W,
+                       void* stream);
 
 #ifdef __cplusplus
 }

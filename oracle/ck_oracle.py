@@ -192,3 +192,21 @@ def waste(attempts, P):
         mx = max(unit)
         out.append(1.0 - float(sum(unit)) / (float(len(unit)) * float(mx)) if mx > 0 else 0.0)
     return np.array(out, dtype=np.float64)
+
+
+def waste_tasks(attempts, P, tasks):
+    """Eq. 20 with `tasks` reactors per lane (the several-tasks-per-thread mitigation the paper cites from ref. [48],
+    PAPER.md:419), written out: unit j = P * tasks consecutive reactors, lane l owns reactors l, l + P, l + 2P, ... of the
+    unit, cost_l = sum of their attempts, W_j = 1 - sum_i N_i / (lanes * max_l cost_l), lanes = lanes owning >= 1 reactor.
+    tasks = 1 is waste().  Pins (tests/test_oracle_waste.py): reduces to waste() at tasks = 1; equal counts -> 0;
+    averaging: W(tasks) of iid counts falls as tasks grows; a unit made of `tasks` copies of one pattern has the W of
+    that pattern."""
+    a = [int(v) for v in np.asarray(attempts).ravel()]
+    per = P * tasks
+    out = []
+    for b in range(0, len(a), per):
+        unit = a[b:b + per]
+        cost = [sum(unit[l::P]) for l in range(min(P, len(unit)))]
+        mx = max(cost)
+        out.append(1.0 - float(sum(unit)) / (float(len(cost)) * float(mx)) if mx > 0 else 0.0)
+    return np.array(out, dtype=np.float64)

@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_waste"):
+                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks"):
             getattr(L, name).restype = C.c_int32
         _lib = L
     return _lib
@@ -158,6 +158,11 @@ class Mechanism:
         except Exception:
             pass
 
+    def rhs_kernel_name(self, n):
+        b, t = C.c_int32(0), C.c_int32(0)
+        _check(lib().ck_rhs_variant(self.h, C.c_int64(n), C.byref(b), C.byref(t)))
+        return f"ck::rhs_kernel_tmem<{b.value}>" if t.value else f"ck::rhs_kernel<{b.value}>"
+
     def rhs_slots(self):
         v = C.c_double(0)
         _check(lib().ck_rhs_slots(self.h, C.byref(v)))
@@ -222,13 +227,14 @@ class Mechanism:
                     ws=ws)
 
     @staticmethod
-    def waste(n_accept, n_reject, P):
-        """Eq. 20 per work unit of width P (static mapping) from device step counts; returns a device tensor."""
+    def waste(n_accept, n_reject, P, tasks=1):
+        """Eq. 20 per work unit of width P (static mapping, `tasks` reactors per lane) from device step counts."""
         import torch
         n = n_accept.numel()
-        W = torch.empty((n + P - 1) // P if P > 0 else 0, dtype=torch.float64, device=n_accept.device)
-        _check(lib().ck_waste(C.c_int64(n), _ptr(n_accept), _ptr(n_reject) if n_reject is not None else None, int(P),
-                              _ptr(W), _stream()))
+        per = P * tasks
+        W = torch.empty((n + per - 1) // per if per > 0 else 0, dtype=torch.float64, device=n_accept.device)
+        _check(lib().ck_waste_tasks(C.c_int64(n), _ptr(n_accept), _ptr(n_reject) if n_reject is not None else None, int(P),
+                                    int(tasks), _ptr(W), _stream()))
         return W
 
     # ---- host-pointer entry points (numpy arrays; transfers inside the call) ---------------------------

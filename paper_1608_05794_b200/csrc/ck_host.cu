@@ -60,6 +60,9 @@ extern "C" int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream
   return CK_OK;
 }
 
+// Chunked pipeline: the batch is column-separable, PCIe is full duplex, so the states are cut into column blocks
+// that travel H2D / through the kernel / D2H on three streams -- while block c is evaluated, block c + 1 is on its way
+// in and block c - 1 on its way out.  Host buffers should be pinned (pageable memory makes the copies synchronous).
 extern "C" int32_t ck_rhs_host(ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* dydt,
                                int64_t ld_out) {
   if (!m) { set_error("ck_rhs_host: null mechanism"); return CK_EINVAL; }
@@ -67,21 +70,31 @@ extern "C" int32_t ck_rhs_host(ck_mech* m, int64_t n, const double* y, int64_t l
   if (n == 0) return CK_OK;
   if (!y || !p || !dydt) { set_error("ck_rhs_host: null batch pointer"); return CK_EINVAL; }
   CK_CUDA(cudaSetDevice(m->device));
-  if (!m->hstream) CK_CUDA(cudaStreamCreateWithFlags(&m->hstream, cudaStreamNonBlocking));
+  constexpr int NS = 3;
+  for (int i = 0; i < NS; ++i)
+    if (!m->pstream[i]) CK_CUDA(cudaStreamCreateWithFlags(&m->pstream[i], cudaStreamNonBlocking));
   const int N = m->K + 1;
-  const size_t by = al((size_t)N * n * sizeof(double)), bp = al((size_t)n * sizeof(double));
-  int32_t rc = stage_reserve(m, 2 * by + bp);
+  // block width: at least the batch the tensor-memory kernel wants, at most an eighth of the batch
+  const int64_t blk = std::min<int64_t>(n, std::max<int64_t>(65536, (n + 7) / 8));
+  const size_t by = al((size_t)N * blk * sizeof(double)), bp = al((size_t)blk * sizeof(double));
+  int32_t rc = stage_reserve(m, NS * (2 * by + bp));
   if (rc) return rc;
-  double* dy = (double*)m->stage;
-  double* df = (double*)((char*)m->stage + by);
-  double* dp = (double*)((char*)m->stage + 2 * by);
-  cudaStream_t st = m->hstream;
-  CK_CUDA(cudaMemcpy2DAsync(dy, n * sizeof(double), y, ld * sizeof(double), n * sizeof(double), N, cudaMemcpyHostToDevice, st));
-  CK_CUDA(cudaMemcpyAsync(dp, p, n * sizeof(double), cudaMemcpyHostToDevice, st));
-  rc = ck_rhs(m, n, dy, n, dp, df, n, st);
-  if (rc) return rc;
-  CK_CUDA(cudaMemcpy2DAsync(dydt, ld_out * sizeof(double), df, n * sizeof(double), n * sizeof(double), N, cudaMemcpyDeviceToHost, st));
-  CK_CUDA(cudaStreamSynchronize(st));
+  int c = 0;
+  for (int64_t b = 0; b < n; b += blk, ++c) {
+    const int64_t nb = std::min<int64_t>(blk, n - b);
+    const int sidx = c % NS;
+    cudaStream_t st = m->pstream[sidx];
+    char* base = (char*)m->stage + (size_t)sidx * (2 * by + bp);
+    double* dy = (double*)base;
+    double* df = (double*)(base + by);
+    double* dp = (double*)(base + 2 * by);
+    CK_CUDA(cudaMemcpy2DAsync(dy, nb * sizeof(double), y + b, ld * sizeof(double), nb * sizeof(double), N, cudaMemcpyHostToDevice, st));
+    CK_CUDA(cudaMemcpyAsync(dp, p + b, nb * sizeof(double), cudaMemcpyHostToDevice, st));
+    rc = ck_rhs(m, nb, dy, nb, dp, df, nb, st);
+    if (rc) return rc;
+    CK_CUDA(cudaMemcpy2DAsync(dydt + b, ld_out * sizeof(double), df, nb * sizeof(double), nb * sizeof(double), N, cudaMemcpyDeviceToHost, st));
+  }
+  for (int i = 0; i < NS; ++i) CK_CUDA(cudaStreamSynchronize(m->pstream[i]));
   return CK_OK;
 }
 

@@ -86,6 +86,7 @@ struct ck_mech {
   void* stage = nullptr;
   size_t stage_bytes = 0;
   cudaStream_t hstream = nullptr;
+  cudaStream_t pstream[3] = {nullptr, nullptr, nullptr};   // column-block pipeline of ck_rhs_host
 };
 
 #define CK_CUDA(call)                                                    \

@@ -341,6 +341,7 @@ extern "C" int32_t ck_mech_free(ck_mech* m) {
   if (m->arena) cudaFree(m->arena);
   if (m->stage) cudaFree(m->stage);
   if (m->hstream) cudaStreamDestroy(m->hstream);
+  for (auto& ps : m->pstream) if (ps) cudaStreamDestroy(ps);
   delete m;
   return CK_OK;
 }

@@ -99,3 +99,13 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
   set_error("ck_rhs: %d species do not fit the shared-memory columns (unsupported)", m->K);
   return CK_EUNSUPPORTED;
 }
+
+// which kernel ck_rhs launches for a batch of n states: CTA width, and whether the production-rate accumulators live
+// in tensor memory (for the roofline record of bench.py: the kernel name comes from the dispatch, not from a constant)
+extern "C" int32_t ck_rhs_variant(const ck_mech* m, int64_t n, int32_t* block, int32_t* tmem) {
+  if (!m || !block || !tmem) { set_error("ck_rhs_variant: null argument"); return CK_EINVAL; }
+  const int b = ck::rhs_tmem_block(m, n);
+  *tmem = b != 0;
+  *block = b ? b : rhs_pick_block(m->K, m->dev.rstride, n);
+  return CK_OK;
+}

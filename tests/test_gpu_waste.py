@@ -22,6 +22,9 @@ def test_waste_matches_oracle_bit_exact(oracle, P, n):
     assert W.shape == ref.shape and np.array_equal(W, ref)
     W1 = ck.Mechanism.waste(torch.from_numpy(na).cuda(), None, P).cpu().numpy()   # n_reject may be null
     assert np.array_equal(W1, oracle.waste(na, P))
+    for tasks in (2, 7):                                                            # several reactors per lane
+        Wt = ck.Mechanism.waste(torch.from_numpy(na).cuda(), torch.from_numpy(nr).cuda(), P, tasks=tasks).cpu().numpy()
+        assert np.array_equal(Wt, oracle.waste_tasks(na.astype(np.int64) + nr, P, tasks))
 
 
 def test_waste_of_a_real_run_and_report_agree(oracle):
