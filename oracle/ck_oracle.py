@@ -61,7 +61,8 @@ def _u8(a):
 
 
 class Mech:
-    def __init__(self, d, variant=None):
+    def __init__(self, d, variant=None, const_volume=False):
+        """const_volume: the `p` argument of every call is then the mass density rho."""
         L = self._L = lib(variant)
         self.K, self.R, self.E = int(d["n_species"]), int(d["n_reactions"]), int(d["n_elements"])
         self.N = self.K + 1
@@ -80,6 +81,8 @@ class Mech:
             _p(k["A"]), _p(k["beta"]), _p(k["Ea"]), _p(k["rev"], C.c_uint8), _p(k["type"], C.c_uint8),
             _p(k["A0"]), _p(k["beta0"]), _p(k["Ea0"]), _p(k["troe"]),
             _p(k["eptr"], C.c_int), _p(k["espec"], C.c_int), _p(k["eval"])))
+        if const_volume:
+            L.cko_set_const_volume(self.h, 1)
 
     def __del__(self):
         try:

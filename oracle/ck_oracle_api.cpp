@@ -49,6 +49,7 @@ void* cko_mech_create(int K, int R, int E, const double* W, const int* elem, con
   return m;
 }
 void cko_mech_free(void* h) { delete (Mech*)h; }
+void cko_set_const_volume(void* h, int on) { ((Mech*)h)->const_volume = on ? 1 : 0; }
 
 // prec 0: double, 1: long double (result rounded to double).  D (optional) = cancellation-aware scale.
 void cko_rhs(void* h, long long n, const double* y, long long ld, const double* p, double* f, long long ldf,

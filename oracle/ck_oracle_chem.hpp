@@ -40,6 +40,9 @@ struct Mech {
   std::vector<double> troe;              // [R*4] a, T***, T*, T** (T**<0: absent)
   std::vector<int> eptr, espec;          // CSR non-unit efficiencies
   std::vector<double> eval;
+  // 0: constant pressure (Eq. 12-13; the argument `p` of rhs is the pressure).  1: constant volume ("rho is
+  // constant ... replacing c_p with c_v and h_k with u_k in Eq. (13)"); the argument `p` of rhs is then the mass density.
+  int const_volume = 0;
 };
 
 // ---- scalar helpers -----------------------------------------------------------------------
@@ -110,7 +113,8 @@ void rhs(const Mech& m, const S* y, double p, S* f, RhsAux* aux = nullptr) {
   // (2) ideal gas: rho = p / (R_u T sum Y_k/W_k); C_k = rho Y_k / W_k
   S Ssum(0.0);
   for (int k = 0; k < K; ++k) Ssum = Ssum + y[1 + k] / S(m.W[k]);
-  const S rho = S(p) / (S(R_U) * T * Ssum);
+  // constant volume: rho is the given constant and the pressure follows from the same equation of state
+  const S rho = m.const_volume ? S(p) : S(p) / (S(R_U) * T * Ssum);
   for (int k = 0; k < K; ++k) C[k] = rho * y[1 + k] / S(m.W[k]);
   if (aux) { aux->qf.assign(R, 0.0); aux->qr.assign(R, 0.0); }
   // (3) reactions in index order
@@ -168,7 +172,15 @@ void rhs(const Mech& m, const S* y, double p, S* f, RhsAux* aux = nullptr) {
     hw = hw + hRT[k] * w[k];
   }
   cp = S(R_U) * cp;
-  f[0] = -(S(R_U) * T * hw) / (rho * cp);
+  if (m.const_volume) {
+    // u_k = h_k - R_u T / W_k (molar: U_k/(R_u T) = H_k/(R_u T) - 1);  c_v = c_p - R_u sum_k Y_k / W_k
+    S uw(0.0);
+    for (int k = 0; k < K; ++k) uw = uw + (hRT[k] - S(1.0)) * w[k];
+    const S cv = cp - S(R_U) * Ssum;
+    f[0] = -(S(R_U) * T * uw) / (rho * cv);
+  } else {
+    f[0] = -(S(R_U) * T * hw) / (rho * cp);
+  }
   if (aux) {
     aux->rho = re(rho); aux->cp = re(cp);
     std::vector<double> Dw(K, 0.0);
@@ -183,9 +195,9 @@ void rhs(const Mech& m, const S* y, double p, S* f, RhsAux* aux = nullptr) {
     double dT = 0;
     for (int k = 0; k < K; ++k) {
       aux->D[1 + k] = m.W[k] / re(rho) * Dw[k];
-      dT += std::fabs(R_U * re(T) * re(hRT[k])) * Dw[k];
+      dT += std::fabs(R_U * re(T) * (re(hRT[k]) - (m.const_volume ? 1.0 : 0.0))) * Dw[k];
     }
-    aux->D[0] = dT / (re(rho) * re(cp));
+    aux->D[0] = dT / (re(rho) * (m.const_volume ? re(cp) - R_U * re(Ssum) : re(cp)));
   }
 }
 
