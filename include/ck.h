@@ -34,6 +34,7 @@ enum { CK_OK = 0, CK_EINVAL = 1, CK_ECUDA = 2, CK_EWORKSPACE = 3, CK_EUNSUPPORTE
 enum { CK_OP_ROS = 0, CK_OP_RKF45 = 1, CK_OP_JAC = 2 };                 /* ck_workspace_bytes `op` */
 enum { CK_PLAIN = 0, CK_THREE_BODY = 1, CK_LINDEMANN = 2, CK_TROE = 3 }; /* ck_mech_desc.type */
 enum { CK_JAC_ANALYTIC = 0, CK_JAC_FD = 1 };
+enum { CK_CONST_PRESSURE = 0, CK_CONST_VOLUME = 1 };                    /* ck_mech_set_reactor `kind` */
 /* per-reactor status written by ck_integrate_* */
 enum { CK_ST_OK = 0, CK_ST_MAX_STEPS = 1, CK_ST_H_UNDERFLOW = 2, CK_ST_NONFINITE = 3, CK_ST_ZERO_PIVOT = 4 };
 
@@ -102,6 +103,12 @@ int32_t ck_version(void);
 int32_t ck_mech_load(const ck_mech_desc* desc, int32_t device, ck_mech** out);
 int32_t ck_mech_free(ck_mech* m);
 int32_t ck_mech_sizes(const ck_mech* m, int32_t* n_species, int32_t* n_reactions);
+/* Reactor kind the handle's compute calls model (default CK_CONST_PRESSURE, Eq. 12-13).  CK_CONST_VOLUME (PAPER.md:107:
+ * "a constant-volume process, i.e., where rho is constant, can be modeled by replacing c_p with c_v and h_k with u_k in
+ * Eq. (13)"): the mass density of each reactor is fixed and the `p` argument of ck_rhs / ck_jac* / ck_integrate_* then
+ * holds that density rho[n] in g/cm^3 instead of the pressure (the pressure follows from p = rho R_u T sum_k Y_k/W_k).
+ * Not thread-safe against compute calls running on the same handle; load a second handle to use both kinds at once. */
+int32_t ck_mech_set_reactor(ck_mech* m, int32_t kind);
 
 /* Scratch bytes ck_integrate_{ros,rkf45} / ck_jac_batched need for n reactors (op = CK_OP_*). */
 int32_t ck_workspace_bytes(const ck_mech* m, int32_t op, int64_t n, size_t* bytes);

@@ -62,7 +62,7 @@ def lib():
         path = _build.build()
         L = C.CDLL(path)
         L.ck_last_error.restype = C.c_char_p
-        for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_workspace_bytes", "ck_rhs", "ck_jac",
+        for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_mech_set_reactor", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
                      "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks"):
             getattr(L, name).restype = C.c_int32
@@ -122,7 +122,8 @@ def lu_solve_batched(A, b):
 class Mechanism:
     """A kinetic model loaded on one GPU.  `d` is a dict whose keys mirror ck_mech_desc."""
 
-    def __init__(self, d, device=0):
+    def __init__(self, d, device=0, const_volume=False):
+        """const_volume: constant-volume reactors -- every `p` argument then holds the mass density (include/ck.h)."""
         L = lib()
         k = self._keep = dict(
             mol_wt=_np(d["mol_wt"], np.float64), elem_comp=_np(d["elem_comp"], np.int32),
@@ -143,6 +144,8 @@ class Mechanism:
         h = C.c_void_p()
         _check(L.ck_mech_load(C.byref(desc), int(device), C.byref(h)))
         self.h = h
+        if const_volume:
+            _check(L.ck_mech_set_reactor(h, 1))
         self.device = int(device)
         self.K, self.R = desc.n_species, desc.n_reactions
         self.N = self.K + 1

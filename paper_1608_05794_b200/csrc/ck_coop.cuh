@@ -100,9 +100,11 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
   const int K = m.K, R = m.R, tid = threadIdx.x;
   t = make_tstate(m, y[0]);
   double Sp = 0.0, cp = 0.0;
+  const double sub = m.cv ? 1.0 : 0.0;
   for (int k = tid; k < K; k += G) {
     double cpR, hRT;
     thermo_cp_h(m, k, t, cpR, hRT);
+    cpR -= sub; hRT -= sub;   // constant volume: c_v,k / R = c_p,k / R - 1, U_k / (R T) = H_k / (R T) - 1
     const double yw = y[1 + k] * __ldg(m.invW + k);
     c.cpR[k] = cpR; c.hRT[k] = hRT; c.yw[k] = yw;
     Sp += yw;
@@ -111,8 +113,8 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
   CoopScalars s;
   s.S = block_sum<G>(Sp, c.red);
   s.cps = block_sum<G>(cp, c.red);
-  s.Ctot = p / (R_U * t.T);
-  s.rho = s.Ctot / s.S;
+  s.rho = m.cv ? p : (p / (R_U * t.T)) / s.S;   // constant volume: `p` is the density
+  s.Ctot = m.cv ? s.rho * s.S : p / (R_U * t.T);
   for (int k = tid; k < K; k += G) c.C[k] = s.rho * c.yw[k];
   if (tid == 0) c.C[K] = 1.0;
   __syncthreads();
@@ -191,9 +193,10 @@ __device__ __forceinline__ void rhs_wide(const MechDev& m, const double* __restr
       tt.T = T; tt.invT = 1.0 / T; tt.lnT = 0.0; tt.tint = 0;
       double cpR, hRT;
       thermo_cp_h(m, tid, tt, cpR, hRT);
+      const double sub = m.cv ? 1.0 : 0.0;   // constant volume: c_v,k and u_k (see rhs_coop)
       yw = y[1 + tid] * __ldg(m.invW + tid);
-      c.hRT[tid] = hRT;
-      cp = yw * cpR;
+      c.hRT[tid] = hRT - sub;
+      cp = yw * (cpR - sub);
     }
     double S = yw;
 #pragma unroll
@@ -204,7 +207,8 @@ __device__ __forceinline__ void rhs_wide(const MechDev& m, const double* __restr
   double S = 0.0, cps = 0.0;
   for (int w = 0; w < KW; ++w) { S += c.red[w]; cps += c.red[8 + w]; }
   t.T = T; t.lnT = c.red[32]; t.invT = c.red[33]; t.tint = (int)c.red[34];
-  const double Ctot = p * t.invT * (1.0 / R_U), rho = Ctot / S;
+  const double rho = m.cv ? p : (p * t.invT * (1.0 / R_U)) / S;
+  const double Ctot = m.cv ? rho * S : p * t.invT * (1.0 / R_U);
   if (tid < K) c.C[tid] = rho * yw;
   if (tid == 0) c.C[K] = 1.0;
   __syncthreads();
@@ -266,9 +270,11 @@ __device__ __forceinline__ CoopScalars rhs_jac_coop(const MechDev& m, const doub
   const int K = m.K, R = m.R, N = K + 1, tid = threadIdx.x;
   t = make_tstate(m, y[0]);
   double Sp = 0.0, cp = 0.0;
+  const double sub = m.cv ? 1.0 : 0.0;
   for (int k = tid; k < K; k += G) {
     double cpR, hRT;
     thermo_cp_h(m, k, t, cpR, hRT);
+    cpR -= sub; hRT -= sub;   // constant volume: c_v,k / R = c_p,k / R - 1, U_k / (R T) = H_k / (R T) - 1
     const double yw = y[1 + k] * __ldg(m.invW + k);
     c.cpR[k] = cpR; c.hRT[k] = hRT; c.yw[k] = yw;
     Sp += yw;
@@ -278,8 +284,8 @@ __device__ __forceinline__ CoopScalars rhs_jac_coop(const MechDev& m, const doub
   CoopScalars s;
   s.S = block_sum<G>(Sp, c.red);
   s.cps = block_sum<G>(cp, c.red);
-  s.Ctot = p / (R_U * t.T);
-  s.rho = s.Ctot / s.S;
+  s.rho = m.cv ? p : (p / (R_U * t.T)) / s.S;   // constant volume: `p` is the density
+  s.Ctot = m.cv ? s.rho * s.S : p / (R_U * t.T);
   for (int k = tid; k < K; k += G) c.C[k] = s.rho * c.yw[k];
   if (tid == 0) c.C[K] = 1.0;
   __syncthreads();
@@ -395,10 +401,13 @@ __device__ __forceinline__ void jac_coop_finish(const MechDev& m, const CoopChem
                                          const double* __restrict__ f, double* __restrict__ A, int lda) {
   const int K = m.K, tid = threadIdx.x;
   // scalars of the temperature row
+  // constant volume: rho does not depend on y, so every term that came from d rho / d y (the sigma terms, f_k / T,
+  // f_k / (S W_j), one of the two f_T / T) drops out: sg = 0; c.cpR / c.hRT / s.cps already hold c_v and u (rhs_coop)
+  const double sg = m.cv ? 0.0 : 1.0;
   double hs = 0.0, ht = 0.0, hcw = 0.0, dcp = 0.0;
   for (int k = tid; k < K; k += G) {
-    hs = fma(c.hRT[k], c.sig[k], hs);
-    ht = fma(c.hRT[k], c.tau[k] - c.sig[k] * t.invT, ht);
+    hs = fma(c.hRT[k], sg * c.sig[k], hs);
+    ht = fma(c.hRT[k], c.tau[k] - sg * c.sig[k] * t.invT, ht);
     hcw = fma((c.cpR[k] - c.hRT[k]) * t.invT, c.w[k], hcw);
     dcp = fma(c.yw[k], thermo_dcp(m, k, t), dcp);
   }
@@ -413,9 +422,9 @@ __device__ __forceinline__ void jac_coop_finish(const MechDev& m, const CoopChem
     double col = 0.0;
     for (int k = 0; k < K; ++k) col = fma(c.hRT[k], A[(size_t)(1 + k) * lda + 1 + j] + c.dns[k], col);
     const double iWj = __ldg(m.invW + j);
-    A[1 + j] = -phi * (s.rho * iWj * col - hs * iS * iWj) + fT * (iS * iWj - c.cpR[j] * iWj / s.cps);
+    A[1 + j] = -phi * (s.rho * iWj * col - hs * iS * iWj) + fT * (sg * iS * iWj - c.cpR[j] * iWj / s.cps);
   }
-  if (tid == 0) A[0] = -phi * (hcw + ht) + fT * (2.0 * t.invT - dcp / s.cps);
+  if (tid == 0) A[0] = -phi * (hcw + ht) + fT * ((1.0 + sg) * t.invT - dcp / s.cps);
   __syncthreads();
   // species rows: in-place transform of G into d f_k / d Y_j, and the temperature column
   const double irho = 1.0 / s.rho;
@@ -423,10 +432,10 @@ __device__ __forceinline__ void jac_coop_finish(const MechDev& m, const CoopChem
     const int k = idx / K, j = idx - k * K;
     const double Wk = __ldg(m.W + k), iWj = __ldg(m.invW + j);
     double* a = A + (size_t)(1 + k) * lda + 1 + j;
-    *a = Wk * iWj * (*a + c.dns[k]) + (f[1 + k] - Wk * irho * c.sig[k]) * iS * iWj;
+    *a = Wk * iWj * (*a + c.dns[k]) + sg * (f[1 + k] - Wk * irho * c.sig[k]) * iS * iWj;
   }
   for (int k = tid; k < K; k += G)
-    A[(size_t)(1 + k) * lda] = __ldg(m.W + k) * irho * (c.tau[k] - c.sig[k] * t.invT) + f[1 + k] * t.invT;
+    A[(size_t)(1 + k) * lda] = __ldg(m.W + k) * irho * (c.tau[k] - sg * c.sig[k] * t.invT) + sg * f[1 + k] * t.invT;
   __syncthreads();
 }
 

@@ -27,6 +27,7 @@ constexpr double T_SAFE_LO = 250.0, T_SAFE_HI = 4500.0;  // window in which the 
 // accumulator at K), so rate products and the omega scatter are branch-free.
 struct MechDev {
   int K, R, nT;
+  int cv;                     // 1: constant-volume reactors: the batch argument `p` holds the density rho
   int r_22;                   // leading rows of the plain group with at most two reactants and two products, all
                               //   distinct (A + B <=> C + D; a missing partner is the dummy species K)
   int r_dup, r_tb, r_lind, r_troe;

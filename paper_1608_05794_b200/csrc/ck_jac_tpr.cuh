@@ -119,7 +119,7 @@ __device__ __forceinline__ void jac_phaseA_row(const MechDev& m, int r, const do
     g2[(size_t)(4 * r) * ldg] = a.ci * a.kf;
     g2[(size_t)(4 * r + 1) * ldg] = a.ci * a.kr;
     g2[(size_t)(4 * r + 2) * ldg] = si;
-    g2[(size_t)(4 * r + 3) * ldg] = fma(-si, t.invT, dqT);
+    g2[(size_t)(4 * r + 3) * ldg] = m.cv ? dqT : fma(-si, t.invT, dqT);   // d C_m / d T = 0 at constant volume
   }
 }
 
@@ -153,8 +153,9 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
       tm_st2(wt + 2 * (k0 + j), 0.0);
     }
   }
-  const double Ctot = p / (R_U * t.T);
-  const double rho = Ctot / S;
+  const double rho = m.cv ? p : (p / (R_U * t.T)) / S;   // constant volume (m.cv): `p` is the density
+  const double Ctot = m.cv ? rho * S : p / (R_U * t.T);
+  const double sub = m.cv ? 1.0 : 0.0, sg = m.cv ? 0.0 : 1.0;   // see jac_coop_finish (ck_coop.cuh)
 #pragma unroll 4
   for (int k = 0; k < K; ++k) Cs[k * BLOCK] *= rho;
   Cs[K * BLOCK] = 1.0;
@@ -178,7 +179,7 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
     for (; j < j3; ++j) jac_phaseA_row<BLOCK, 2>(m, r0 + j, stage + j * rs, xs + 16 * j, t, Cs, Ctot, wt, g2, o.ldg, store);
     for (; j < nr; ++j) jac_phaseA_row<BLOCK, 3>(m, r0 + j, stage + j * rs, xs + 16 * j, t, Cs, Ctot, wt, g2, o.ldg, store);
   }
-  const double irho = 1.0 / rho, icps = 1.0 / cps;
+  const double irho = 1.0 / rho, icps = 1.0 / (cps - sub * S);   // c_v / R = c_p / R - S at constant volume
   double hw = 0.0;
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
@@ -190,12 +191,12 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
       double w;
       tm_ld2(wt + 2 * (k0 + j), w);
       tm_wait_ld();
-      const double hrt = thermo_row_h(row, t);
+      const double hrt = thermo_row_h(row, t) - sub;
       hw = fma(hrt, w, hw);
       if (store) {
         fout[(size_t)(k0 + j + 1) * o.ldf] = w * row[0] * irho;
         hc[(size_t)(k0 + j) * o.ldh] = t.T * hrt * row[1] * icps;            // hh_k = T (H_k/RT) / (W_k cps)
-        hc[(size_t)(K + k0 + j) * o.ldh] = thermo_row_cp(row, t) * row[1] * icps;  // cc_k = (cp_k/R) / (W_k cps)
+        hc[(size_t)(K + k0 + j) * o.ldh] = (thermo_row_cp(row, t) - sub) * row[1] * icps;  // cc_k = (cp_k/R) / (W_k cps)
       }
     }
   }
@@ -327,8 +328,8 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
     //                           J_kT = (W_k / rho) Theta_k + f_k / T,  Theta_k = sum_i nu_ki theta_i
     const double Wk = sW[k];
     const double fk = store ? fout[(size_t)(1 + k) * o.ldf] : 0.0;
-    const double beta = fma(Wk, dns, (fk - Wk * irho * sig) * iS);
-    const double JkT = fma(Wk * irho, tht, fk * t.invT);
+    const double beta = fma(Wk, dns, sg * (fk - Wk * irho * sig) * iS);
+    const double JkT = fma(Wk * irho, tht, sg * fk * t.invT);
     if (store) sfc = fma(fk, hc[(size_t)(K + k) * o.ldh], sfc);
     for (int c0 = 0; c0 < NP; c0 += 4) {
       double v[4];

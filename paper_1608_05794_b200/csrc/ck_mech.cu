@@ -314,7 +314,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   m->arena_bytes = a.buf.size();
   const char* base = (const char*)m->arena;
   MechDev& v = m->dev;
-  v.K = K; v.R = R; v.nT = nT;
+  v.K = K; v.R = R; v.nT = nT; v.cv = 0;
   v.t_safe_lo = T_SAFE_LO; v.t_safe_hi = T_SAFE_HI;
   v.r_tbf = r_tb + n_tbf;
   v.r_22 = r_22; v.r_dup = r_dup; v.r_tb = r_tb; v.r_lind = r_lind; v.r_troe = r_troe;
@@ -343,6 +343,12 @@ extern "C" int32_t ck_mech_free(ck_mech* m) {
   if (m->hstream) cudaStreamDestroy(m->hstream);
   for (auto& ps : m->pstream) if (ps) cudaStreamDestroy(ps);
   delete m;
+  return CK_OK;
+}
+
+extern "C" int32_t ck_mech_set_reactor(ck_mech* m, int32_t kind) {
+  if (!m || (kind != CK_CONST_PRESSURE && kind != CK_CONST_VOLUME)) { set_error("ck_mech_set_reactor: bad argument"); return CK_EINVAL; }
+  m->dev.cv = (kind == CK_CONST_VOLUME) ? 1 : 0;
   return CK_OK;
 }
 

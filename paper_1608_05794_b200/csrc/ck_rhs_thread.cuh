@@ -84,8 +84,9 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
       ws[(k0 + j) * BLOCK] = 0.0;
     }
   }
-  const double Ctot = p / (R_U * t.T);  // = rho * S
-  const double rho = Ctot / S;
+  // constant pressure: rho = p / (R_u T S); constant volume (m.cv): `p` IS rho; Ctot = sum_k C_k = rho S either way
+  const double rho = m.cv ? p : (p / (R_U * t.T)) / S;
+  const double Ctot = m.cv ? rho * S : p / (R_U * t.T);
 #pragma unroll 4
   for (int k = 0; k < K; ++k) Cs[k * BLOCK] *= rho;
   Cs[K * BLOCK] = 1.0;
@@ -133,6 +134,7 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
   }
   // (4) Eq. 12-13 (13 in reading G2)
   const double irho = 1.0 / rho;
+  const double sub = m.cv ? 1.0 : 0.0;   // constant volume: u_k / (R_u T) = H_k / (R_u T) - 1 and c_v / R_u = c_p / R_u - S
   double hw = 0.0;
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
@@ -143,11 +145,11 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
     for (int j = 0; j < nk; ++j) {
       const double* row = stage + j * SPS;
       const double w = ws[(k0 + j) * BLOCK];
-      hw = fma(thermo_row_h(row, t), w, hw);
+      hw = fma(thermo_row_h(row, t) - sub, w, hw);
       if (store) fout[(size_t)(k0 + j + 1) * ldout] = w * row[0] * irho;
     }
   }
-  if (store) fout[0] = -(t.T * hw) / (rho * cps);  // R_u cancels: -R_u T hw / (rho R_u cps)
+  if (store) fout[0] = -(t.T * hw) / (rho * (cps - sub * S));  // R_u cancels: -R_u T hw / (rho R_u cps)
 }
 
 // largest block whose columns fit in shared memory, halved while the grid would leave most SMs idle

@@ -168,8 +168,9 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
       tm_st2(wt + 2 * (k0 + j), 0.0);
     }
   }
-  const double Ctot = p / (R_U * t.T);
-  const double rho = Ctot / S;
+  // constant pressure: rho = p / (R_u T S); constant volume (m.cv): `p` IS rho; Ctot = sum_k C_k = rho S either way
+  const double rho = m.cv ? p : (p / (R_U * t.T)) / S;
+  const double Ctot = m.cv ? rho * S : p / (R_U * t.T);
 #pragma unroll 4
   for (int k = 0; k < K; ++k) Cs[k * BLOCK] *= rho;
   Cs[K * BLOCK] = 1.0;
@@ -201,6 +202,7 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
     for (; j < nr; ++j) slow_rows_tmem<BLOCK, 3, 1>(m, r0 + j, stage + j * rs, rs, xs + 16 * j, t, Cs, Ctot, wt);
   }
   const double irho = 1.0 / rho;
+  const double sub = m.cv ? 1.0 : 0.0;   // constant volume: u_k / (R_u T) = H_k / (R_u T) - 1 and c_v / R_u = c_p / R_u - S
   double hw = 0.0;
   for (int k0 = 0; k0 < K; k0 += RHS_CHUNK) {
     const int nk = min(RHS_CHUNK, K - k0);
@@ -218,12 +220,12 @@ __device__ __forceinline__ void rhs_thread_tmem(const MechDev& m, const double* 
         if (j0 + u < nk) {
           const double* row = stage + (j0 + u) * SPS;
           const double w = __hiloint2double((int)hi[u], (int)lo[u]);
-          hw = fma(thermo_row_h(row, t), w, hw);
+          hw = fma(thermo_row_h(row, t) - sub, w, hw);
           if (store) fout[(size_t)(k0 + j0 + u + 1) * ldout] = w * row[0] * irho;
         }
     }
   }
-  if (store) fout[0] = -(t.T * hw) / (rho * cps);
+  if (store) fout[0] = -(t.T * hw) / (rho * (cps - sub * S));
 }
 
 // tensor-memory columns a CTA of `block` threads allocates: one set of 2 (K+1) per group of four warps, rounded up to
