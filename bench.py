@@ -288,6 +288,31 @@ def rhs_extras(torch, ck, dev, steps=10):
     return out
 
 
+def run_case(args):
+    """One plain invocation of one workload, for profiler captures (profiles/*.md name these command lines):
+    --case rhs | C1 | C3 | C4 | C5 | C6 | C7 [--case-flags F] runs config 2's ck_rhs three times, resp. one integration."""
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+    dev = torch.device("cuda", 0)
+    name = "C2" if args.case == "rhs" else args.case
+    mech, y, p, cfg = make_config(name)
+    M = ck.Mechanism(mech, device=0)
+    yd = torch.from_numpy(y).to(dev); pd = torch.from_numpy(p).to(dev)
+    if args.case == "rhs":
+        out = torch.empty_like(yd)
+        for _ in range(3):
+            M.rhs(yd, pd, out=out)
+        torch.cuda.synchronize()
+        print(json.dumps({"case": "rhs", "kernel": M.rhs_kernel_name(y.shape[1]), "n": int(y.shape[1])}))
+        return
+    e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+    e0.record()
+    res = M.integrate(cfg["call"], yd, pd, cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"], flags=args.case_flags)
+    e1.record(); torch.cuda.synchronize()
+    print(json.dumps({"case": args.case, "flags": args.case_flags, "ms_first_call": e0.elapsed_time(e1), "report": res["report"]}))
+
+
 def run_ours(args):
     import torch
     import paper_1608_05794_b200 as ck
@@ -396,8 +421,13 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--extras", type=int, default=1, help="also time the integrators on configs 1,3,4,5 (rank 0, N=1)")
+    ap.add_argument("--extras", type=int, default=1, help="also time the integrators on configs 1,3-7 (rank 0, N=1)")
+    ap.add_argument("--case", default=None, help="profiling aid: run ONE workload once (rhs, C1, C3..C7) and exit")
+    ap.add_argument("--case-flags", type=int, default=0, help="ck_opts.flags for --case")
     args = ap.parse_args()
+    if args.case:
+        run_case(args)
+        return
     if args.impl == "reference":
         run_reference(args)
     else:

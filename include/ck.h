@@ -102,6 +102,18 @@ int32_t ck_version(void);
  * species on one side of a reaction or more than 8 distinct t_mid values. */
 int32_t ck_mech_load(const ck_mech_desc* desc, int32_t device, ck_mech** out);
 int32_t ck_mech_free(ck_mech* m);
+
+/* Kinetic model from CHEMKIN-II style text (ELEMENTS / SPECIES / THERMO with four-card NASA-7 entries / REACTIONS with
+ * "<=>", "=", "=>", "+M", "(+M)", LOW/, TROE/, efficiencies, DUPLICATE; '!' comments; cm-mol-s-K, cal/mol): the
+ * counterpart of the paper's `create_rate_subs` interpreter.  Host code, no device needed.  The
+ * returned object owns the arrays ck_parsed_desc() points to; pass that description to ck_mech_load, then free it.
+ * ck_parsed_name: species (what = 0) or element (what = 1) name number `index`.  CK_EINVAL with a line number in
+ * ck_last_error() on malformed input. */
+typedef struct ck_parsed ck_parsed;
+int32_t ck_mech_parse(const char* text, ck_parsed** out);
+const ck_mech_desc* ck_parsed_desc(const ck_parsed* p);
+int32_t ck_parsed_name(const ck_parsed* p, int32_t what, int32_t index, char* buf, int32_t len);
+int32_t ck_parsed_free(ck_parsed* p);
 int32_t ck_mech_sizes(const ck_mech* m, int32_t* n_species, int32_t* n_reactions);
 /* Reactor kind the handle's compute calls model (default CK_CONST_PRESSURE, Eq. 12-13).  CK_CONST_VOLUME (PAPER.md:107:
  * "a constant-volume process, i.e., where rho is constant, can be modeled by replacing c_p with c_v and h_k with u_k in

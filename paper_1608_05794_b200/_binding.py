@@ -64,8 +64,10 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_mech_set_reactor", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks"):
+                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks", "ck_mech_parse", "ck_parsed_name",
+                     "ck_parsed_free"):
             getattr(L, name).restype = C.c_int32
+        L.ck_parsed_desc.restype = C.POINTER(MechDesc)
         _lib = L
     return _lib
 
@@ -107,6 +109,41 @@ def fp64_peak(device=0):
     v = C.c_double(0)
     _check(lib().ck_fp64_peak(int(device), C.byref(v), None))
     return v.value
+
+
+def parse_mechanism(text):
+    """CHEMKIN-II style text -> dict with the keys of ck_mech_desc (+ species_names, elements), via ck_mech_parse."""
+    L = lib()
+    h = C.c_void_p()
+    _check(L.ck_mech_parse(text.encode(), C.byref(h)))
+    try:
+        d = L.ck_parsed_desc(h).contents
+        K, R, E = d.n_species, d.n_reactions, d.n_elements
+        arr = lambda ptr, n, dt: np.ctypeslib.as_array(ptr, shape=(n,)).astype(dt).copy() if n else np.zeros(0, dt)
+        out = dict(n_species=K, n_reactions=R, n_elements=E,
+                   mol_wt=arr(d.mol_wt, K, np.float64), elem_comp=arr(d.elem_comp, K * E, np.int32).reshape(K, E),
+                   nasa_lo=arr(d.nasa_lo, 7 * K, np.float64).reshape(K, 7), nasa_hi=arr(d.nasa_hi, 7 * K, np.float64).reshape(K, 7),
+                   t_mid=arr(d.t_mid, K, np.float64), reac_ptr=arr(d.reac_ptr, R + 1, np.int32), prod_ptr=arr(d.prod_ptr, R + 1, np.int32),
+                   eff_ptr=arr(d.eff_ptr, R + 1, np.int32), A=arr(d.A, R, np.float64), beta=arr(d.beta, R, np.float64),
+                   Ea=arr(d.Ea, R, np.float64), reversible=arr(d.reversible, R, np.uint8), type=arr(d.type, R, np.uint8),
+                   A0=arr(d.A0, R, np.float64), beta0=arr(d.beta0, R, np.float64), Ea0=arr(d.Ea0, R, np.float64),
+                   troe=arr(d.troe, 4 * R, np.float64).reshape(R, 4))
+        nr, npd, ne = int(out["reac_ptr"][-1]), int(out["prod_ptr"][-1]), int(out["eff_ptr"][-1])
+        out.update(reac_spec=arr(d.reac_spec, nr, np.int32), reac_nu=arr(d.reac_nu, nr, np.int32),
+                   prod_spec=arr(d.prod_spec, npd, np.int32), prod_nu=arr(d.prod_nu, npd, np.int32),
+                   eff_spec=arr(d.eff_spec, ne, np.int32), eff_val=arr(d.eff_val, ne, np.float64))
+        buf = C.create_string_buffer(64)
+        names = []
+        for what, n in ((0, K), (1, E)):
+            lst = []
+            for i in range(n):
+                _check(L.ck_parsed_name(h, what, i, buf, 64))
+                lst.append(buf.value.decode())
+            names.append(lst)
+        out["species_names"], out["elements"] = names
+        return out
+    finally:
+        L.ck_parsed_free(h)
 
 
 def lu_solve_batched(A, b):

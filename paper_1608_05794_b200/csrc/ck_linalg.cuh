@@ -325,102 +325,6 @@ __device__ __forceinline__ bool lu_factor_rows_smem(double* __restrict__ A, int 
   return ok;
 }
 
-// Segmented register-resident factorisation for compile-time N <= G: thread tid < N holds row tid of the matrix in
-// registers (as lu_factor_rows), but the step loop is a RUNTIME loop inside compile-time column segments of length S,
-// so the code is N/S loop bodies instead of N unrolled steps (the fully unrolled variant is instruction-fetch
-// bound).  Inside segment [J0, J0+S) every step updates ALL columns j >= J0 of the register row: columns <= k are
-// dead registers by then (their multipliers were stored to shared memory when they were computed), so whatever the
-// update leaves there is never read.  The rank-1 update therefore costs one broadcast shared-memory load per FMA
-// instead of two loads and a store, which is what bounded lu_factor_rows_smem (shared-memory pipe).
-// Publishing the pivot row: after the warp stage of the pivot search, each warp's own best candidate row copies its
-// live registers (columns >= k) to its shared-memory row BEFORE the cross-warp exchange, so one barrier per step
-// serves both the exchange and the row; a warp candidate that loses has only refreshed dead storage.
-// Layout on return is that of lu_factor_rows_smem: A[i][k] = multiplier for k < pstep_i, U beyond, dinv[k] = 1/U_kk.
-// x if i == j else y, opaque to the optimiser: written as a C++ conditional over the columns of the register row,
-// nvcc recognises the chain as a dynamically indexed array read and moves the whole row to local memory.
-__device__ __forceinline__ double sel_eq_f64(int i, int j, double x, double y) {
-  double r;
-  asm("{\n\t.reg .pred p;\n\tsetp.eq.s32 p, %1, %2;\n\tselp.f64 %0, %3, %4, p;\n\t}" : "=d"(r) : "r"(i), "r"(j), "d"(x), "d"(y));
-  return r;
-}
-
-template <int N, int G, int S, int J0>
-__device__ __forceinline__ void lu_factor_seg(double (&a)[N], int& pstep, double& cand, double& cinv, double* __restrict__ A,
-                                              int lda, double* __restrict__ dinv, double* red2, bool& ok) {
-  if constexpr (J0 < N) {
-    constexpr int J1 = (J0 + S < N) ? J0 + S : N;
-    constexpr int W = G / 32;
-    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    double* row = A + (size_t)(tid < N ? tid : 0) * lda;
-#pragma unroll 1
-    for (int k = J0; k < J1; ++k) {
-      const double v = (pstep == -1) ? fabs(cand) : -1.0;
-      const unsigned hi = (v >= 0.0 || v != v) ? (unsigned)__double2hiint(fabs(v)) + 1u : 0u;
-      const unsigned lo = (unsigned)__double2loint(v);
-      const unsigned mh = __reduce_max_sync(0xffffffffu, hi);
-      const unsigned lo2 = (hi == mh) ? lo : 0u;
-      const unsigned ml = __reduce_max_sync(0xffffffffu, lo2);
-      const unsigned win = __ballot_sync(0xffffffffu, hi == mh && lo2 == ml);
-      const int wl = __ffs(win) - 1;
-      if (lane == wl && pstep == -1) {
-#pragma unroll
-        for (int j = J0; j < N; ++j)
-          if (j >= J1 || j >= k) row[j] = a[j];
-      }
-      int p = (w << 5) + wl;
-      double ipv = __shfl_sync(0xffffffffu, cinv, wl);
-      if constexpr (W == 1) {
-        __syncwarp();
-      } else {
-        double* base = red2 + (k & 1) * 4 * W;
-        unsigned* rk = reinterpret_cast<unsigned*>(base);  // [W][2] keys
-        int* ri = reinterpret_cast<int*>(base + W);        // [W] rows
-        double* rinv = base + 2 * W;                       // [W] reciprocals
-        if (lane == 0) { rk[2 * w] = mh; rk[2 * w + 1] = ml; ri[w] = p; rinv[w] = ipv; }
-        __syncthreads();
-        unsigned bh = rk[0], bl = rk[1];
-        p = ri[0]; ipv = rinv[0];
-#pragma unroll
-        for (int i = 1; i < W; ++i) {
-          const unsigned h2 = rk[2 * i], l2 = rk[2 * i + 1];
-          if (h2 > bh || (h2 == bh && l2 > bl)) { bh = h2; bl = l2; p = ri[i]; ipv = rinv[i]; }
-        }
-      }
-      if (!isfinite(ipv) || ipv == 0.0) ok = false;  // zero / non-finite pivot (uniform)
-      const double* prow = A + (size_t)p * lda;
-      // straight-line update (two warps per CTA: a taken branch costs more than the work it skips).  Rows that are
-      // out (pivot rows, tid >= N) run the FMAs on dead registers; only the stores are predicated.
-      const bool upd = (pstep == -1) && (tid != p);
-      if (tid == p) dinv[k] = ipv;
-      pstep = (tid == p) ? k : pstep;
-      const double l = cand * ipv;
-      if (upd) row[k] = l;
-#pragma unroll
-      for (int j = J0; j < N; ++j) a[j] = fma(-l, prow[j], a[j]);
-      if constexpr (J0 + 1 < N) {  // next step's candidate: column k+1, somewhere in (J0, J1]
-        double c = a[J0 + 1];
-#pragma unroll
-        for (int j = J0 + 2; j <= J1 && j < N; ++j) c = sel_eq_f64(k + 1, j, a[j], c);
-        cand = upd ? c : 1.0;  // rows that are out keep a harmless candidate (no slow path in the reciprocal)
-        cinv = 1.0 / cand;
-      }
-    }
-    lu_factor_seg<N, G, S, J1>(a, pstep, cand, cinv, A, lda, dinv, red2, ok);
-  }
-}
-
-// a: this thread's row (thread tid < N owns row tid; zeros for tid >= N).  red2: 2 x 4 x (G/32) doubles.
-template <int N, int G, int S>
-__device__ __forceinline__ bool lu_factor_rows_seg(double (&a)[N], int& pstep, double* __restrict__ A, int lda,
-                                                   double* __restrict__ dinv, double* red2) {
-  pstep = (threadIdx.x < N) ? -1 : -2;
-  bool ok = true;
-  double cand = a[0], cinv = 1.0 / a[0];
-  lu_factor_seg<N, G, S, 0>(a, pstep, cand, cinv, A, lda, dinv, red2, ok);
-  __syncthreads();
-  return ok;
-}
-
 // b: entry `tid` of the right-hand side on entry, x[pstep] on return.  bs: 2 doubles of shared scratch.
 template <int G>
 __device__ __forceinline__ void lu_solve_rows_smem(const double* __restrict__ A, int lda, int N, int pstep,

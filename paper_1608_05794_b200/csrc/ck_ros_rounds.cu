@@ -6,16 +6,17 @@
 // evaluations per attempt -- runs CTA-cooperatively at ~4 k SM-cycles per evaluation, against ~0.7 k for the
 // thread-per-reactor tensor-memory kernel of ck_rhs.  Here the chemistry runs thread-per-reactor over the whole active
 // list (ck_rhs itself and jac_rows_kernel, ck_jac_tpr.cuh); only what is genuinely per-reactor dense linear algebra --
-// the LU factorisation of I/(h gamma) - J and the four stage solves of Eq. 6 -- stays cooperative,
-// with the matrix streamed in from HBM once per attempt.  One attempt round:
+// the LU factorisation of I/(h gamma) - J and the four stage solves of Eq. 6 -- stays cooperative
+// (ck_lu_warp.cuh: blocked, trailing update on the FP64 tensor cores, right-hand sides by shuffle), with the matrix
+// streamed in from HBM once per attempt.  One attempt round:
 //
 //   gather     Yw[:, s] = y[:, act[s]]                                              (thread per slot)
 //   jac_rows   f0 = f(Yw), species rows of J, pieces of row 0        -> F0, LU buffer, HC     (thread per slot)
-//   lu         row 0, A = I/(h gamma) - J, P A = L U, u1 = A^-1 f0, YT = y + a21 u1           (CTA per slot)
+//   lu         row 0, A = I/(h gamma) - J, P A = L U, u1 = A^-1 f0, YT = y + a21 u1           (2-4 warps per slot)
 //   ck_rhs     FT = f(YT)                                                                     (thread per slot)
-//   solve2     u2 = A^-1 (FT + c21/h u1), YT = y + a31 u1 + a32 u2                            (CTA per slot)
+//   solve2     u2 = A^-1 (FT + c21/h u1), YT = y + a31 u1 + a32 u2                            (2-4 warps per slot)
 //   ck_rhs     FT = f(YT)
-//   solve34    u3, u4, y*, error, accept / reject, new h (Algorithm 1), re-queue   (CTA per slot)
+//   solve34    u3, u4, y*, error, accept / reject, new h (Algorithm 1), re-queue   (2-4 warps per slot)
 //
 // Reactors that reached t_f or failed leave the list; the next round runs on the survivors, compacted.  When few
 // are left the round's fixed latency (one thread-per-reactor wave) dominates, so the tail is re-batched once more:
@@ -25,9 +26,7 @@
 #include <cstdlib>
 #include <vector>
 
-#include "ck_coop.cuh"
 #include "ck_jac_tpr.cuh"
-#include "ck_linalg.cuh"
 #include "ck_lu_warp.cuh"
 #include "ck_ros_common.cuh"
 
@@ -56,7 +55,7 @@ struct RoundArgs {
   long long lu_stride;
   int lu_ldr;
   double* dinv;                    // [cap][N]
-  int* pst;                        // [cap][N] elimination step at which a row was the pivot
+  int* pst;                        // [cap][N] row permutation of the factorisation
   double* hs;                      // [cap] step size of this attempt
   int* flg;                        // [cap] bit 0: clipped to t_f, bit 1: zero pivot
   DevStats* stats;
@@ -132,219 +131,6 @@ __global__ void ros_guard_kernel(RoundArgs a) {
 }
 __global__ void ros_swap_kernel(RoundArgs a) { a.cnt[0] = a.cnt[1]; a.cnt[1] = 0; }
 
-// ---- cooperative kernels: CTA of G threads per slot, thread i owns matrix row i ---------------------------------
-__host__ __device__ inline int rr_lda(int N) { return N | 1; }
-__host__ __device__ inline size_t rr_smem_doubles(int N) { return (size_t)N * rr_lda(N) + 12 * (size_t)N + 64; }
-
-struct RrShared { double *A, *e, *Lb, *Ub, *v0, *v1, *v2, *v3, *red; };
-__device__ __forceinline__ RrShared rr_carve(double* sm, int N) {
-  RrShared s;
-  s.A = sm; sm += (size_t)N * rr_lda(N);
-  s.e = sm; sm += N;
-  s.Lb = sm; sm += 3 * N; s.Ub = sm; sm += 3 * N;
-  s.v0 = sm; sm += N; s.v1 = sm; sm += N; s.v2 = sm; sm += N; s.v3 = sm; sm += N;
-  s.red = sm + N;
-  return s;
-}
-
-// factors (L\U rows, 1/U_kk, pivot steps) between shared memory and the slot's block in HBM
-template <int G>
-__device__ __forceinline__ void rr_store_factors(const RoundArgs& a, long long s, int N, const RrShared& sh, int pstep) {
-  const int NP = a.lu_ldr, lda = rr_lda(N), tid = threadIdx.x;
-  double* dst = a.LU + (size_t)s * a.lu_stride;
-  for (int idx = tid; idx < N * NP; idx += G) {
-    const int i = idx / NP, j = idx - i * NP;
-    dst[idx] = (j < N) ? sh.A[(size_t)i * lda + j] : 0.0;
-  }
-  for (int i = tid; i < N; i += G) a.dinv[(size_t)s * N + i] = sh.e[i];
-  if (tid < N) a.pst[(size_t)s * N + tid] = pstep;
-}
-template <int G>
-__device__ __forceinline__ int rr_load_factors(const RoundArgs& a, long long s, int N, const RrShared& sh) {
-  const int NP = a.lu_ldr, lda = rr_lda(N), tid = threadIdx.x;
-  const double* src = a.LU + (size_t)s * a.lu_stride;
-  for (int idx = tid; idx < N * NP; idx += G) {
-    const int i = idx / NP, j = idx - i * NP;
-    if (j < N) sh.A[(size_t)i * lda + j] = src[idx];
-  }
-  for (int i = tid; i < N; i += G) sh.e[i] = a.dinv[(size_t)s * N + i];
-  const int pstep = (tid < N) ? a.pst[(size_t)s * N + tid] : -2;
-  __syncthreads();
-  lu_compact4<G>(sh.A, lda, N, pstep, sh.Lb, sh.Ub);
-  return pstep;
-}
-// x = A^-1 b with b[tid] in `bb`; the solution lands in x_out (shared, indexed by component)
-template <int G>
-__device__ __forceinline__ void rr_solve(const RrShared& sh, int N, int pstep, double bb, double* __restrict__ x_out) {
-  lu_solve_rows_blk<G>(sh.A, rr_lda(N), N, pstep, sh.e, sh.Lb, sh.Ub, bb, sh.red);
-  if (pstep >= 0) x_out[pstep] = bb;
-  __syncthreads();
-}
-
-// NS > 0: compile-time N with the rows in registers during the factorisation (lu_factor_rows_seg); NS < 0: any N <= G
-template <int G, int NS>
-__global__ void __launch_bounds__(G) ros_lu_kernel(RoundArgs a, int K) {
-  using namespace ros4c;
-  extern __shared__ double sm[];
-  const int N = K + 1, lda = rr_lda(N), NP = a.lu_ldr, tid = threadIdx.x;
-  const RrShared sh = rr_carve(sm, N);
-  const long long na = a.cnt[0];
-  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
-    const int r = a.act[s];
-    __syncthreads();
-    // species rows of J (written by jac_rows_kernel) and the vectors that give row 0 (ck_jac_tpr.cuh)
-    const double* src = a.LU + (size_t)s * a.lu_stride;
-    for (int idx = tid + NP; idx < N * NP; idx += G) {
-      const int i = idx / NP, j = idx - i * NP;
-      if (j < N) sh.A[(size_t)i * lda + j] = src[idx];
-    }
-    for (int k = tid; k < K; k += G) { sh.v0[k] = a.HC[(size_t)k * a.cap + s]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + s]; }
-    for (int i = tid; i < N; i += G) sh.v2[i] = a.F0[(size_t)i * a.cap + s];
-    __syncthreads();
-    const double fT = sh.v2[0];
-    for (int j = tid; j < N; j += G) {
-      double acc = 0.0;
-      for (int k = 0; k < K; ++k) acc = fma(sh.v0[k], sh.A[(size_t)(1 + k) * lda + j], acc);
-      sh.A[j] = (j == 0) ? (a.HC[(size_t)(2 * K) * a.cap + s] - acc) : (-acc - fT * sh.v1[j - 1]);
-    }
-    // step size of this attempt: clip to t_f (Algorithm 1)
-    double h = a.h[r];
-    const double trem = a.dt - a.t[r];
-    int flg = 0;
-    if (h >= trem) { h = trem; flg = 1; }
-    const double ihg = 1.0 / (h * gam);
-    __syncthreads();
-    bool ok;
-    int pstep = -2;
-    if constexpr (NS > 0) {  // A = I/(h gamma) - J formed while the rows are loaded into registers
-      double arow[NS];
-      if (tid < NS) {
-#pragma unroll
-        for (int j = 0; j < NS; ++j) arow[j] = -sh.A[(size_t)tid * lda + j] + (j == tid ? ihg : 0.0);
-      } else {
-#pragma unroll
-        for (int j = 0; j < NS; ++j) arow[j] = 0.0;
-      }
-      __syncthreads();
-      ok = lu_factor_rows_seg<NS, G, 9>(arow, pstep, sh.A, lda, sh.e, sh.red);
-    } else {
-      for (int idx = tid; idx < N * lda; idx += G) sh.A[idx] = -sh.A[idx];
-      __syncthreads();
-      for (int i = tid; i < N; i += G) sh.A[(size_t)i * lda + i] += ihg;
-      __syncthreads();
-      ok = lu_factor_rows_smem<G>(sh.A, lda, N, pstep, sh.e, sh.red);
-    }
-    if (!ok) flg |= 2;
-    lu_compact4<G>(sh.A, lda, N, pstep, sh.Lb, sh.Ub);
-    rr_store_factors<G>(a, s, N, sh, pstep);
-    rr_solve<G>(sh, N, pstep, (tid < N) ? sh.v2[tid] : 0.0, sh.v3);   // u1 = A^-1 f0
-    for (int i = tid; i < N; i += G) {
-      const double u1 = sh.v3[i];
-      a.U1[(size_t)s * N + i] = u1;
-      a.YT[(size_t)i * a.cap + s] = fma(a21, u1, a.Yw[(size_t)i * a.cap + s]);
-    }
-    if (tid == 0) { a.hs[s] = h; a.flg[s] = flg; }
-  }
-}
-
-template <int G>
-__global__ void __launch_bounds__(G) ros_solve2_kernel(RoundArgs a, int K) {
-  using namespace ros4c;
-  extern __shared__ double sm[];
-  const int N = K + 1, tid = threadIdx.x;
-  const RrShared sh = rr_carve(sm, N);
-  const long long na = a.cnt[0];
-  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
-    __syncthreads();
-    for (int i = tid; i < N; i += G) sh.v0[i] = a.U1[(size_t)s * N + i];
-    const int pstep = rr_load_factors<G>(a, s, N, sh);
-    const double ih = 1.0 / a.hs[s];
-    const double bb = (tid < N) ? fma(c21 * ih, sh.v0[tid], a.FT[(size_t)tid * a.cap + s]) : 0.0;
-    rr_solve<G>(sh, N, pstep, bb, sh.v1);   // u2
-    for (int i = tid; i < N; i += G) {
-      const double u2 = sh.v1[i];
-      a.U2[(size_t)s * N + i] = u2;
-      a.YT[(size_t)i * a.cap + s] = a.Yw[(size_t)i * a.cap + s] + a31 * sh.v0[i] + a32 * u2;
-    }
-  }
-}
-
-template <int G>
-__global__ void __launch_bounds__(G) ros_solve34_kernel(RoundArgs a, int K) {
-  using namespace ros4c;
-  extern __shared__ double sm[];
-  const int N = K + 1, tid = threadIdx.x;
-  const RrShared sh = rr_carve(sm, N);
-  const long long na = a.cnt[0];
-  unsigned long long c_acc = 0, c_rej = 0, c_fail = 0;
-  for (long long s = blockIdx.x; s < na; s += gridDim.x) {
-    const int r = a.act[s];
-    __syncthreads();
-    for (int i = tid; i < N; i += G) { sh.v0[i] = a.U1[(size_t)s * N + i]; sh.v1[i] = a.U2[(size_t)s * N + i]; }
-    const int pstep = rr_load_factors<G>(a, s, N, sh);
-    const double h = a.hs[s], ih = 1.0 / h;
-    const int flg = a.flg[s];
-    const double ft = (tid < N) ? a.FT[(size_t)tid * a.cap + s] : 0.0;
-    double bb = (tid < N) ? ft + (c31 * sh.v0[tid] + c32 * sh.v1[tid]) * ih : 0.0;
-    rr_solve<G>(sh, N, pstep, bb, sh.v2);   // u3
-    bb = (tid < N) ? ft + (c41 * sh.v0[tid] + c42 * sh.v1[tid] + c43 * sh.v2[tid]) * ih : 0.0;
-    rr_solve<G>(sh, N, pstep, bb, sh.v3);   // u4
-    double es = 0.0, yn = 0.0;
-    if (tid < N) {
-      const double y0 = a.Yw[(size_t)tid * a.cap + s];
-      const double u1 = sh.v0[tid], u2 = sh.v1[tid], u3 = sh.v2[tid], u4 = sh.v3[tid];
-      yn = y0 + m1 * u1 + m2 * u2 + m3 * u3 + m4 * u4;
-      const double e = e1 * u1 + e2 * u2 + e3 * u3 + e4 * u4;
-      const double w = e / fma(a.rtol, fmax(fabs(y0), fabs(yn)), a.atol);
-      es = w * w;
-    }
-    const double err = sqrt(block_sum<G>(es, sh.red) / N);
-    // ---- accept / reject, new h (Algorithm 1; controller of DESIGN.md reading G8) -- uniform across the CTA
-    double tcur = a.t[r], hn = h, fac_max = a.fac[r];
-    int nacc = a.nacc[r], nrej = a.nrej[r], status = CK_ST_OK;
-    bool done = false;
-    if (flg & 2) { status = CK_ST_ZERO_PIVOT; done = true; }
-    else if (isfinite(err) && err < 1.0) {
-      if (tid < N) a.y[(size_t)tid * a.ld + r] = yn;
-      tcur = (flg & 1) ? a.dt : tcur + h;
-      nacc++;
-      hn = h * fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25)));
-      fac_max = 5.0;
-      c_acc++;
-    } else {
-      nrej++;
-      hn = h * (isfinite(err) ? fmin(1.0, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25))) : 0.2);
-      fac_max = 1.0;
-      c_rej++;
-    }
-    if (!done) {
-      if (!(tcur < a.dt)) done = true;
-      else if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; done = true; }
-      else if (!isfinite(hn)) { status = CK_ST_NONFINITE; done = true; }
-      else if (hn < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; done = true; }
-    }
-    if (tid == 0) {
-      a.t[r] = tcur; a.h[r] = hn; a.fac[r] = fac_max; a.nacc[r] = nacc; a.nrej[r] = nrej;
-      if (done) {
-        if (a.n_accept) a.n_accept[r] = nacc;
-        if (a.n_reject) a.n_reject[r] = nrej;
-        if (a.status) a.status[r] = status;
-        if (a.h_last) a.h_last[r] = (flg & 2) ? 0.0 : h;
-        a.att[r] = nacc + nrej;
-        c_fail += (status != CK_ST_OK);
-      } else {
-        a.act2[atomicAdd(&a.cnt[1], 1)] = r;
-      }
-    }
-  }
-  if (tid == 0) {
-    atomicAdd(&a.stats->attempts, c_acc + c_rej);
-    atomicAdd(&a.stats->accepted, c_acc);
-    atomicAdd(&a.stats->rejected, c_rej);
-    atomicAdd(&a.stats->failed, c_fail);
-  }
-}
-
 // ---- warp-per-reactor kernels: blocked DMMA LU and shuffle solves (ck_lu_warp.cuh); CTA = one warp = one slot ------
 // The slot's block in HBM is the shared-memory image of the matrix (luw_np(N) rows of stride luw_lda(N)): it moves
 // as a flat vector copy.  pst[] holds the row permutation.
@@ -361,8 +147,8 @@ __device__ __forceinline__ RwShared rw_carve(double* sm, int N) {
   s.perm = reinterpret_cast<int*>(sm);
   return s;
 }
-constexpr int RW = 2;          // warps per CTA: warp 0 runs the serial chains, all warps the parallel phases
-constexpr int RWT = 32 * RW;
+// RW warps per CTA: warp 0 runs the serial chains (panel steps, solves), all warps the parallel phases
+template <int RWT>
 __device__ __forceinline__ void rw_copy_block(double* __restrict__ dst, const double* __restrict__ src, int doubles) {
   const int tid = threadIdx.x;
   const double2* s2 = reinterpret_cast<const double2*>(src);
@@ -371,16 +157,17 @@ __device__ __forceinline__ void rw_copy_block(double* __restrict__ dst, const do
 #pragma unroll 8
   for (int i = tid; i < n2; i += RWT) d2[i] = s2[i];
 }
-template <int NR>
+template <int RWT>
 __device__ __forceinline__ void rw_load_factors(const RoundArgs& a, long long s, int N, const RwShared& sh) {
   const int tid = threadIdx.x;
-  rw_copy_block(sh.A, a.LU + (size_t)s * a.lu_stride, luw_block_doubles(N));
+  rw_copy_block<RWT>(sh.A, a.LU + (size_t)s * a.lu_stride, luw_block_doubles(N));
   for (int i = tid; i < N; i += RWT) { sh.dinv[i] = a.dinv[(size_t)s * N + i]; sh.perm[i] = a.pst[(size_t)s * N + i]; }
 }
 
-template <int NR>
-__global__ void __launch_bounds__(RWT) ros_lu_w_kernel(RoundArgs a, int K) {
+template <int NR, int RW>
+__global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
   using namespace ros4c;
+  constexpr int RWT = 32 * RW;
   extern __shared__ double sm[];
   __shared__ int s_ok;
   const int N = K + 1, lda = luw_lda(N), NP = luw_np(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -396,9 +183,9 @@ __global__ void __launch_bounds__(RWT) ros_lu_w_kernel(RoundArgs a, int K) {
       const double2* src2 = reinterpret_cast<const double2*>(blk);
 #pragma unroll 4
       for (int i = 1 + warp; i < N; i += RW) {
-        if (lane < h2) {
-          const double2 v = src2[(size_t)i * h2 + lane];
-          double* d = sh.A + (size_t)i * lda + 2 * lane;
+        for (int c = lane; c < h2; c += 32) {
+          const double2 v = src2[(size_t)i * h2 + c];
+          double* d = sh.A + (size_t)i * lda + 2 * c;
           d[0] = -v.x; d[1] = -v.y;
         }
       }
@@ -435,7 +222,7 @@ __global__ void __launch_bounds__(RWT) ros_lu_w_kernel(RoundArgs a, int K) {
     if (tid == 0) s_ok = ok ? 1 : 0;
     __syncthreads();
     if (!s_ok) flg |= 2;
-    rw_copy_block(blk, sh.A, luw_block_doubles(N));
+    rw_copy_block<RWT>(blk, sh.A, luw_block_doubles(N));
     for (int i = tid; i < N; i += RWT) { a.dinv[(size_t)s * N + i] = sh.dinv[i]; a.pst[(size_t)s * N + i] = sh.perm[i]; }
     if (warp == 0) {
       double bb[NR];
@@ -455,16 +242,17 @@ __global__ void __launch_bounds__(RWT) ros_lu_w_kernel(RoundArgs a, int K) {
   }
 }
 
-template <int NR>
-__global__ void __launch_bounds__(RWT) ros_solve2_w_kernel(RoundArgs a, int K) {
+template <int NR, int RW>
+__global__ void __launch_bounds__(32 * RW) ros_solve2_w_kernel(RoundArgs a, int K) {
   using namespace ros4c;
+  constexpr int RWT = 32 * RW;
   extern __shared__ double sm[];
   const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const RwShared sh = rw_carve(sm, N);
   const long long na = a.cnt[0];
   for (long long s = blockIdx.x; s < na; s += gridDim.x) {
     __syncthreads();
-    rw_load_factors<NR>(a, s, N, sh);
+    rw_load_factors<RWT>(a, s, N, sh);
     const double ih = 1.0 / a.hs[s];
     for (int i = tid; i < N; i += RWT) {
       const double u1 = a.U1[(size_t)s * N + i];
@@ -489,9 +277,10 @@ __global__ void __launch_bounds__(RWT) ros_solve2_w_kernel(RoundArgs a, int K) {
   }
 }
 
-template <int NR>
-__global__ void __launch_bounds__(RWT) ros_solve34_w_kernel(RoundArgs a, int K) {
+template <int NR, int RW>
+__global__ void __launch_bounds__(32 * RW) ros_solve34_w_kernel(RoundArgs a, int K) {
   using namespace ros4c;
+  constexpr int RWT = 32 * RW;
   extern __shared__ double sm[];
   const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const RwShared sh = rw_carve(sm, N);
@@ -500,7 +289,7 @@ __global__ void __launch_bounds__(RWT) ros_solve34_w_kernel(RoundArgs a, int K) 
   for (long long s = blockIdx.x; s < na; s += gridDim.x) {
     const int r = a.act[s];
     __syncthreads();
-    rw_load_factors<NR>(a, s, N, sh);
+    rw_load_factors<RWT>(a, s, N, sh);
     const double h = a.hs[s], ih = 1.0 / h;
     const int flg = a.flg[s];
     double u1[NR], u2[NR], ft[NR], y0[NR];
@@ -599,13 +388,10 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
 
 namespace {
 inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
-inline int rr_group(int N) { return N <= 32 ? 32 : (N <= 64 ? 64 : 128); }
-// warp-per-reactor LU / solves (ck_lu_warp.cuh) where a matrix block is small enough for several warps per SM
-inline bool rr_use_warp(const ck_mech* m) { return m->K + 1 <= 64; }
 inline int rr_lu_ldr(const ck_mech* m) { return jac_np(m->K + 1); }   // row stride of the species rows of J in a slot's block
 inline long long rr_lu_stride(const ck_mech* m) {
   const int N = m->K + 1;
-  return rr_use_warp(m) ? (long long)luw_block_doubles(N) : (long long)N * jac_np(N);
+  return (long long)luw_block_doubles(N);
 }
 
 struct RrLayout {
@@ -644,33 +430,9 @@ int32_t launch_jac_rows_rm(const ck_mech* m, const RoundArgs& a, long long na, i
   return CK_OK;
 }
 
-template <int G, int NS>
-int32_t launch_coop(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
-  const int N = m->K + 1;
-  const size_t smem = rr_smem_doubles(N) * sizeof(double);
-  int per_sm = 0;
-  if (which == 0) {
-    CK_CUDA(cudaFuncSetAttribute(ros_lu_kernel<G, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_lu_kernel<G, NS>, G, smem));
-    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
-    ros_lu_kernel<G, NS><<<(unsigned)grid, G, smem, st>>>(a, m->K);
-  } else if (which == 1) {
-    CK_CUDA(cudaFuncSetAttribute(ros_solve2_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_solve2_kernel<G>, G, smem));
-    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
-    ros_solve2_kernel<G><<<(unsigned)grid, G, smem, st>>>(a, m->K);
-  } else {
-    CK_CUDA(cudaFuncSetAttribute(ros_solve34_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ros_solve34_kernel<G>, G, smem));
-    const long long grid = std::max<long long>(1, std::min<long long>(na, (long long)std::max(per_sm, 1) * sms));
-    ros_solve34_kernel<G><<<(unsigned)grid, G, smem, st>>>(a, m->K);
-  }
-  CK_CUDA(cudaGetLastError());
-  return CK_OK;
-}
-
-template <int NR>
+template <int NR, int RW>
 int32_t launch_warp(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
+  constexpr int RWT = 32 * RW;
   const int N = m->K + 1;
   const size_t smem = rw_smem_bytes(N);
   int per_sm = 0;
@@ -682,19 +444,17 @@ int32_t launch_warp(const ck_mech* m, const RoundArgs& a, long long na, int sms,
     CK_CUDA(cudaGetLastError());
     return CK_OK;
   };
-  if (which == 0) return go(ros_lu_w_kernel<NR>);
-  if (which == 1) return go(ros_solve2_w_kernel<NR>);
-  return go(ros_solve34_w_kernel<NR>);
+  if (which == 0) return go(ros_lu_w_kernel<NR, RW>);
+  if (which == 1) return go(ros_solve2_w_kernel<NR, RW>);
+  return go(ros_solve34_w_kernel<NR, RW>);
 }
 
 int32_t coop_dispatch(const ck_mech* m, const RoundArgs& a, long long na, int sms, int which, cudaStream_t st) {
   const int N = m->K + 1;
-  if (rr_use_warp(m)) return (N <= 32) ? launch_warp<1>(m, a, na, sms, which, st) : launch_warp<2>(m, a, na, sms, which, st);
-  switch (rr_group(N)) {
-    case 32: return launch_coop<32, -1>(m, a, na, sms, which, st);
-    case 64: return launch_coop<64, -1>(m, a, na, sms, which, st);
-    default: return launch_coop<128, -1>(m, a, na, sms, which, st);
-  }
+  if (N <= 32) return launch_warp<1, 2>(m, a, na, sms, which, st);
+  if (N <= 64) return launch_warp<2, 2>(m, a, na, sms, which, st);
+  if (N <= 96) return launch_warp<3, 4>(m, a, na, sms, which, st);
+  return launch_warp<4, 4>(m, a, na, sms, which, st);
 }
 }  // namespace
 
@@ -703,7 +463,7 @@ namespace ck {
 bool ros_rounds_supported(const ck_mech* m) {
   const int N = m->K + 1;
   return N <= 128 && jac_tpr_block(m->dev) != 0 && m->dev.rstride <= 64 &&
-         (rr_use_warp(m) ? rw_smem_bytes(N) : rr_smem_doubles(N) * sizeof(double)) <= 227 * 1024;
+         rw_smem_bytes(N) <= 227 * 1024;
 }
 size_t ros_rounds_workspace(const ck_mech* m, int64_t n) { return n > 0 ? rr_layout(m, n).total : sizeof(DevStats); }
 
@@ -741,7 +501,7 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   int32_t rc;
   unsigned long long rhs_evals = 0, jac_evals = 0;
   double slots_act = 0, slots_tot = 0;   // lane utilisation: active slots / lanes issued, summed over the launches
-  const int jblock = jac_tpr_block(m->dev), G = rr_use_warp(m) ? 32 * ((N + 31) / 32) : rr_group(N);
+  const int jblock = jac_tpr_block(m->dev), G = 32 * ((N + 31) / 32);
   auto count_tpr = [&](long long na, int block) { slots_act += (double)na; slots_tot += (double)((na + block - 1) / block) * block; };
   ros_init_kernel<<<gn, tb, 0, st>>>(a);
   ros_gather_kernel<<<gn, tb, 0, st>>>(a, N);
@@ -758,8 +518,7 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   std::swap(a.act, a.act2);
   if ((rc = read_count(&na))) return fail(rc);
   // the tail (few survivors: a round costs one thread-per-reactor wave whatever the count) goes to the fused kernel
-  const char* te = getenv("CK_ROS_TAIL");
-  const long long tail = te ? atoll(te) : std::min<long long>(4096, std::max<long long>(n / 8, 1));
+  const long long tail = std::min<long long>(4096, std::max<long long>(n / 8, 1));
   int rounds = 0;
   while (na >= tail && na > 0) {
     const unsigned ga = (unsigned)((na + tb - 1) / tb);

@@ -7,9 +7,9 @@ reactors: once as it stands and once compiled from the SAME sources with fused m
 The explicit solver takes thousands of stability-limited steps on the stiffer reactors, its accept/reject pattern flips
 with the last bit, and the two CPU results differ beyond the literal bound on some trace species -- so no implementation
 can be required to meet that bound entry by entry against either of them.  What is unique is the exact solution; the
-P3 rule (>= 99.9 % of the entries inside the literal bound, and on every other reactor a global error no larger than
-twice the reference's plus one tolerance unit against a tight-tolerance solve) holds between the two CPU builds, and it
-is the rule tests/test_gpu_integrate.py applies to the GPU."""
+P3 rule (>= 99.9 % of the entries inside the literal bound, and every other reactor within north_star's bound of a
+tight-tolerance solve, or with a global error no larger than twice the reference's plus one tolerance unit) holds
+between the two CPU builds, and it is the rule tests/test_gpu_integrate.py applies to the GPU."""
 import numpy as np
 import pytest
 
@@ -53,7 +53,9 @@ def test_two_correct_fp64_executions_violate_the_literal_bound_on_c4(oracle):
         sc = 1e-6 * np.abs(col) + 1e-10
         ea = np.sqrt(np.mean(((ra["y"][:, r] - col) / sc) ** 2))
         eb = np.sqrt(np.mean(((rb["y"][:, r] - col) / sc) ** 2))
-        assert eb <= 2.0 * ea + 1.0 and ea <= 2.0 * eb + 1.0, (int(r), float(ea), float(eb))
+        lim = np.maximum(1e-5 * np.abs(col), np.where(np.arange(col.size) == 0, 0.0, 1e-10))
+        for res, e_this, e_other in ((ra, ea, eb), (rb, eb, ea)):   # the rule the GPU tests apply, both ways round
+            assert np.all(np.abs(res["y"][:, r] - col) <= lim) or e_this <= 2.0 * e_other + 1.0, (int(r), float(ea), float(eb))
 
 
 @pytest.mark.skipif(not _has_fma(), reason="host CPU without FMA: the second build cannot run")
