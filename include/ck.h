@@ -141,6 +141,18 @@ int32_t ck_jac(const ck_mech* m, int64_t n, const double* y, int64_t ld, const d
 int32_t ck_jac_batched(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* J, int64_t ldJ,
                        void* ws, size_t ws_bytes, void* stream);
 
+/* ck_jac_batched for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): same kernels, same output, but the scratch lives in a file-scope device array of CK_JAC_STATIC_BYTES that
+ * every GPU loading the library holds until exit -- no workspace argument, no cudaMalloc / cudaFree inside.
+ * CK_EWORKSPACE (with the limit in ck_last_error()) when n reactors of this model need more scratch than that;
+ * ck_jac_static_max_reactors gives the largest n that fits (2,761 for a 53-species / 325-reaction model, 1,161 for
+ * 111 / 784).  All calls on one device share the array, which keeps the last call's contents (nothing needs clearing:
+ * every entry is written before it is read): calls that OVERLAP on the GPU race -- serialise them on one stream. */
+#define CK_JAC_STATIC_BYTES (32u << 20)
+int32_t ck_jac_batched_static(const ck_mech* m, int64_t n, const double* y, int64_t ld, const double* p, double* J,
+                              int64_t ldJ, void* stream);
+int32_t ck_jac_static_max_reactors(const ck_mech* m, int64_t* n_max);
+
 /* The per-reactor dense linear algebra of the Rosenbrock stage equations on its own (Eq. 6; cost
  * ~ N^3): for each of n systems factor A_r (row-major N x N at A + r N N, not modified) with partial
  * pivoting (first maximal |a| wins ties) and solve A_r x_r = b_r (b, x: [n][N]).  status[r] (optional) = CK_ST_OK or

@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_mech_set_reactor", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks", "ck_mech_parse", "ck_parsed_name",
+                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_jac_batched_static", "ck_jac_static_max_reactors", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks", "ck_mech_parse", "ck_parsed_name",
                      "ck_parsed_free"):
             getattr(L, name).restype = C.c_int32
         L.ck_parsed_desc.restype = C.POINTER(MechDesc)
@@ -239,6 +239,18 @@ class Mechanism:
         _check(lib().ck_jac_batched(self.h, C.c_int64(n), _ptr(y), C.c_int64(y.stride(0) if n else 0), _ptr(p), _ptr(out),
                                     C.c_int64(out.stride(0) if n else 0), _ptr(ws), C.c_size_t(ws.numel()), _stream()))
         return out.view(self.N, self.N, n)
+
+    def jac_batched_static(self, y, p, out):
+        """ck_jac_batched_static: no allocation inside the call; `out` (N*N, n) must be supplied by the caller."""
+        n = y.shape[1]
+        _check(lib().ck_jac_batched_static(self.h, C.c_int64(n), _ptr(y), C.c_int64(y.stride(0) if n else 0), _ptr(p), _ptr(out),
+                                           C.c_int64(out.stride(0) if n else 0), _stream()))
+        return out.view(self.N, self.N, n)
+
+    def jac_static_max_reactors(self):
+        v = C.c_int64(0)
+        _check(lib().ck_jac_static_max_reactors(self.h, C.byref(v)))
+        return v.value
 
     def workspace_bytes(self, op, n):
         v = C.c_size_t(0)

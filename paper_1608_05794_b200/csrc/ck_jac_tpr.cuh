@@ -401,7 +401,7 @@ __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, lon
 }
 
 // Row 0 of a component-major Jacobian from its species rows (see the header): one thread per reactor.
-__global__ void __launch_bounds__(128) jac_trow_kernel(int K, long long n, const double* __restrict__ f, long long ldf,
+static __global__ void __launch_bounds__(128) jac_trow_kernel(int K, long long n, const double* __restrict__ f, long long ldf,
                                                        const double* __restrict__ hc, long long ldh, double* __restrict__ J,
                                                        long long ldJ) {
   const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;

@@ -1,0 +1,49 @@
+"""ck_jac_batched_static: the allocation-free variant of ck_jac_batched (scratch in a file-scope device array of
+CK_JAC_STATIC_BYTES = 32 MiB instead of a caller workspace), for callers that cannot call cudaMalloc.  Checked against
+the existing path on two calls in a row (the array keeps the first call's contents; the second call uses another size
+and another model so that stale contents would show), plus the size limit.  This file is collected last on purpose."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+
+def test_static_scratch_jacobian_matches_workspace_path_twice_and_rejects_oversize():
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+    mech, y, p, _ = make_config("C3", n=1500)
+    M = ck.Mechanism(mech)
+    nmax = M.jac_static_max_reactors()
+    assert 1500 <= nmax < 65536
+    for call, n in enumerate((1500, 777)):                      # two calls in a row, different batch sizes
+        yd = torch.from_numpy(np.ascontiguousarray(y[:, :n])).cuda(); pd = torch.from_numpy(np.ascontiguousarray(p[:n])).cuda()
+        ref = M.jac_batched(yd, pd)                              # existing path (allocates its workspace through torch)
+        out = torch.full((M.N * M.N, n), float("nan"), dtype=torch.float64, device="cuda")
+        free0 = torch.cuda.mem_get_info()[0]
+        got = M.jac_batched_static(yd, pd, out)
+        torch.cuda.synchronize()
+        assert torch.cuda.mem_get_info()[0] == free0            # nothing was allocated on the device by the call
+        a, b = got.cpu().numpy(), ref.cpu().numpy()
+        assert np.isfinite(a).all()
+        # north_star's tolerance for the Jacobian (relative 1e-12 per component); the two paths run the same kernels
+        assert np.all(np.abs(a - b) <= 1e-12 * np.abs(b) + 1e-300), (call, float(np.abs(a - b).max()))
+    # a third call on ANOTHER model right after (different scratch layout over the same array)
+    mech1, y1, p1, _ = make_config("C1", n=2000)
+    M1 = ck.Mechanism(mech1)
+    yd = torch.from_numpy(y1).cuda(); pd = torch.from_numpy(p1).cuda()
+    out = torch.empty((M1.N * M1.N, 2000), dtype=torch.float64, device="cuda")
+    a = M1.jac_batched_static(yd, pd, out).cpu().numpy(); b = M1.jac_batched(yd, pd).cpu().numpy()
+    assert np.all(np.abs(a - b) <= 1e-12 * np.abs(b) + 1e-300)
+    # beyond the maximum: a clear error, nothing launched
+    n_big = nmax + 1
+    yb = torch.from_numpy(np.ascontiguousarray(np.tile(y, (1, n_big // 1500 + 1))[:, :n_big])).cuda()
+    pb = torch.from_numpy(np.ascontiguousarray(np.tile(p, n_big // 1500 + 1)[:n_big])).cuda()
+    ob = torch.empty((M.N * M.N, n_big), dtype=torch.float64, device="cuda")
+    with pytest.raises(ck.CkError) as e:
+        M.jac_batched_static(yb, pb, ob)
+    assert e.value.code == 3 and "at most" in str(e.value) and str(nmax) in str(e.value)
+    # exactly the maximum is accepted
+    got = M.jac_batched_static(yb[:, :nmax], pb[:nmax], ob[:, :nmax])
+    torch.cuda.synchronize()
+    assert torch.isfinite(got).all()
