@@ -123,7 +123,7 @@ __device__ __forceinline__ void jac_phaseA_row(const MechDev& m, int r, const do
   }
 }
 
-// RM: reactor-major output (rows padded to NP), else component-major.  MUST be called by every thread of the CTA.
+// RM: reactor-major output of the NEGATED species rows (row stride o.ldr, o.sstride doubles per slot), else component-major J.  MUST be called by every thread of the CTA.
 // yin / out pointers are pre-offset to this thread's slot (component-major arrays) resp. reactor (Jrm).
 template <int BLOCK, bool RM>
 __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
@@ -331,6 +331,10 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
     const double beta = fma(Wk, dns, sg * (fk - Wk * irho * sig) * iS);
     const double JkT = fma(Wk * irho, tht, sg * fk * t.invT);
     if (store) sfc = fma(fk, hc[(size_t)(K + k) * o.ldh], sfc);
+    double* const rowbase = RM ? o.J + (size_t)(1 + k) * o.ldr : nullptr;
+    // odd row stride (the LU's shared-memory image): every other row starts 8 bytes off a 16-byte boundary
+    const bool odd_row = RM && (o.ldr & 1) && ((1 + k) & 1);
+    double carry = 0.0;
     for (int c0 = 0; c0 < NP; c0 += 4) {
       double v[4];
       tm_ld8(wt + 2 * c0, v);
@@ -342,15 +346,17 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
         v[x] = (cidx == 0) ? JkT : ((cidx <= K) ? siW[j] * fma(Wk, v[x], beta) : 0.0);
       }
       if (store) {
-        if (RM) {
-          double* dst = o.J + (size_t)(1 + k) * o.ldr + c0;
-          if (o.ldr & 1) {  // odd row stride (shared-memory image of the warp LU): rows are only 8-byte aligned
-#pragma unroll
-            for (int x = 0; x < 4; ++x) dst[x] = v[x];
-          } else {
-            reinterpret_cast<double2*>(dst)[0] = make_double2(v[0], v[1]);
-            reinterpret_cast<double2*>(dst)[1] = make_double2(v[2], v[3]);
+        if (RM) {  // rows of -J (what the factorisation of I/(h gamma) - J starts from), in the row stride of the LU's image
+          double* dst = rowbase + c0;
+          if (!odd_row) {
+            reinterpret_cast<double2*>(dst)[0] = make_double2(-v[0], -v[1]);
+            reinterpret_cast<double2*>(dst)[1] = make_double2(-v[2], -v[3]);
+          } else {  // row starts 8 bytes off a 16-byte boundary: pair the last element of a piece with the first of the next
+            if (c0 == 0) dst[0] = -v[0];
+            else *reinterpret_cast<double2*>(dst - 1) = make_double2(carry, -v[0]);
+            *reinterpret_cast<double2*>(dst + 1) = make_double2(-v[1], -v[2]);
           }
+          carry = -v[3];
         } else {
 #pragma unroll
           for (int x = 0; x < 4; ++x)
@@ -358,6 +364,7 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
         }
       }
     }
+    if (store && odd_row) rowbase[NP - 1] = carry;
     tm_wait_st();
   }
   if (store) hc[(size_t)(2 * K) * o.ldh] = -sfc - fT * dcp * icps;

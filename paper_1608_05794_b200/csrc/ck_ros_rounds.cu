@@ -26,6 +26,7 @@
 #include <cstdlib>
 #include <vector>
 
+#include "ck_bulk.cuh"
 #include "ck_jac_tpr.cuh"
 #include "ck_lu_warp.cuh"
 #include "ck_ros_common.cuh"
@@ -157,11 +158,20 @@ __device__ __forceinline__ void rw_copy_block(double* __restrict__ dst, const do
 #pragma unroll 8
   for (int i = tid; i < n2; i += RWT) d2[i] = s2[i];
 }
+// the slot's matrix block -> shared memory as ONE bulk copy (the caller has made sure that nobody still uses sh.A and waits
+// on `bar` with the current parity before reading it)
+__device__ __forceinline__ void rw_issue_block_load(const RoundArgs& a, long long s, int N, const RwShared& sh, uint64_t* bar) {
+  if (threadIdx.x == 0) {
+    fence_async_smem();
+    bulk_load(sh.A, a.LU + (size_t)s * a.lu_stride, (uint32_t)(luw_block_doubles(N) * sizeof(double)), bar);
+  }
+}
 template <int RWT>
-__device__ __forceinline__ void rw_load_factors(const RoundArgs& a, long long s, int N, const RwShared& sh) {
+__device__ __forceinline__ void rw_load_factors(const RoundArgs& a, long long s, int N, const RwShared& sh, uint64_t* bar, uint32_t parity) {
   const int tid = threadIdx.x;
-  rw_copy_block<RWT>(sh.A, a.LU + (size_t)s * a.lu_stride, luw_block_doubles(N));
+  rw_issue_block_load(a, s, N, sh, bar);
   for (int i = tid; i < N; i += RWT) { sh.dinv[i] = a.dinv[(size_t)s * N + i]; sh.perm[i] = a.pst[(size_t)s * N + i]; }
+  mbar_wait(bar, parity);
 }
 
 template <int NR, int RW>
@@ -170,29 +180,19 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
   constexpr int RWT = 32 * RW;
   extern __shared__ double sm[];
   __shared__ int s_ok;
+  __shared__ __align__(8) uint64_t s_bar;
   const int N = K + 1, lda = luw_lda(N), NP = luw_np(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const RwShared sh = rw_carve(sm, N);
   const long long na = a.cnt[0];
+  if (tid == 0) mbar_init(&s_bar, 1);
+  uint32_t parity = 0;
   for (long long s = blockIdx.x; s < na; s += gridDim.x) {
     const int r = a.act[s];
+    if (tid == 0) bulk_store_wait_read();   // the previous slot's factors have left shared memory
     __syncthreads();
     double* blk = a.LU + (size_t)s * a.lu_stride;
-    // species rows of J (stride lu_ldr in HBM, written by jac_rows_kernel) land negated in the padded image
-    {
-      const int h2 = a.lu_ldr >> 1;
-      const double2* src2 = reinterpret_cast<const double2*>(blk);
-#pragma unroll 4
-      for (int i = 1 + warp; i < N; i += RW) {
-        for (int c = lane; c < h2; c += 32) {
-          const double2 v = src2[(size_t)i * h2 + c];
-          double* d = sh.A + (size_t)i * lda + 2 * c;
-          d[0] = -v.x; d[1] = -v.y;
-        }
-      }
-      for (int idx = tid; idx < (NP - N) * lda; idx += RWT) sh.A[(size_t)N * lda + idx] = 0.0;   // padding rows
-      for (int i = tid; i < NP; i += RWT)
-        for (int j = a.lu_ldr; j < lda; ++j) sh.A[(size_t)i * lda + j] = 0.0;                   // padding columns
-    }
+    // the slot's block (rows 1..K of -J, written by jac_rows_kernel in the image's layout) arrives as one bulk copy
+    rw_issue_block_load(a, s, N, sh, &s_bar);
     for (int k = tid; k < K; k += RWT) { sh.v0[k] = a.HC[(size_t)k * a.cap + s]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + s]; }
     for (int i = tid; i < N; i += RWT) sh.v2[i] = a.F0[(size_t)i * a.cap + s];
     double h = a.h[r];
@@ -200,6 +200,12 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
     int flg = 0;
     if (h >= trem) { h = trem; flg = 1; }
     const double ihg = 1.0 / (h * gam);
+    mbar_wait(&s_bar, parity);
+    parity ^= 1u;
+    // padding rows / columns of the image: stale (factors of an earlier round, or never written)
+    for (int idx = tid; idx < (NP - N) * lda; idx += RWT) sh.A[(size_t)N * lda + idx] = 0.0;
+    for (int i = tid; i < NP; i += RWT)
+      for (int j = jac_np(N); j < lda; ++j) sh.A[(size_t)i * lda + j] = 0.0;
     __syncthreads();
     // row 0 of A = I/(h gamma) - J from the (negated) species rows (ck_jac_tpr.cuh): -J_0j = -sum_k hh_k M_kj + f_T cc_j
     const double fT = sh.v2[0];
@@ -222,7 +228,9 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
     if (tid == 0) s_ok = ok ? 1 : 0;
     __syncthreads();
     if (!s_ok) flg |= 2;
-    rw_copy_block<RWT>(blk, sh.A, luw_block_doubles(N));
+    fence_async_smem();      // the factors, written through the generic proxy, become visible to the bulk store
+    __syncthreads();
+    if (tid == 0) bulk_store(blk, sh.A, (uint32_t)(luw_block_doubles(N) * sizeof(double)));
     for (int i = tid; i < N; i += RWT) { a.dinv[(size_t)s * N + i] = sh.dinv[i]; a.pst[(size_t)s * N + i] = sh.perm[i]; }
     if (warp == 0) {
       double bb[NR];
@@ -240,6 +248,7 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
       if (lane == 0) { a.hs[s] = h; a.flg[s] = flg; }
     }
   }
+  if (tid == 0) bulk_store_wait_read();
 }
 
 template <int NR, int RW>
@@ -249,10 +258,14 @@ __global__ void __launch_bounds__(32 * RW) ros_solve2_w_kernel(RoundArgs a, int 
   extern __shared__ double sm[];
   const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const RwShared sh = rw_carve(sm, N);
+  __shared__ __align__(8) uint64_t s_bar;
+  if (threadIdx.x == 0) mbar_init(&s_bar, 1);
+  uint32_t parity = 0;
   const long long na = a.cnt[0];
   for (long long s = blockIdx.x; s < na; s += gridDim.x) {
     __syncthreads();
-    rw_load_factors<RWT>(a, s, N, sh);
+    rw_load_factors<RWT>(a, s, N, sh, &s_bar, parity);
+    parity ^= 1u;
     const double ih = 1.0 / a.hs[s];
     for (int i = tid; i < N; i += RWT) {
       const double u1 = a.U1[(size_t)s * N + i];
@@ -284,12 +297,16 @@ __global__ void __launch_bounds__(32 * RW) ros_solve34_w_kernel(RoundArgs a, int
   extern __shared__ double sm[];
   const int N = K + 1, lda = luw_lda(N), tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const RwShared sh = rw_carve(sm, N);
+  __shared__ __align__(8) uint64_t s_bar;
+  if (threadIdx.x == 0) mbar_init(&s_bar, 1);
+  uint32_t parity = 0;
   const long long na = a.cnt[0];
   unsigned long long c_acc = 0, c_rej = 0, c_fail = 0;
   for (long long s = blockIdx.x; s < na; s += gridDim.x) {
     const int r = a.act[s];
     __syncthreads();
-    rw_load_factors<RWT>(a, s, N, sh);
+    rw_load_factors<RWT>(a, s, N, sh, &s_bar, parity);
+    parity ^= 1u;
     const double h = a.hs[s], ih = 1.0 / h;
     const int flg = a.flg[s];
     double u1[NR], u2[NR], ft[NR], y0[NR];
@@ -388,7 +405,7 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
 
 namespace {
 inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
-inline int rr_lu_ldr(const ck_mech* m) { return jac_np(m->K + 1); }   // row stride of the species rows of J in a slot's block
+inline int rr_lu_ldr(const ck_mech* m) { return luw_lda(m->K + 1); }   // the slot's block is the shared-memory image of the matrix
 inline long long rr_lu_stride(const ck_mech* m) {
   const int N = m->K + 1;
   return (long long)luw_block_doubles(N);
