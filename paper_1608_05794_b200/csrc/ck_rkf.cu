@@ -43,14 +43,20 @@ struct RkfArgs {
   double* h_last;
   int* att;
   // hand-over records of reactors evicted at an attempt boundary (finished by rkf45_coop_kernel)
-  int* elist;           // [n] evicted reactor ids
+  int* elist;           // [n] after the classification phase: reactors to resume (from the front), stragglers (from the back)
+  int* elist2;          // [n] reactors evicted at the end-game (narrow finisher)
   double* rec_t;        // [n] time reached
   double* rec_h;        // [n] next step size
   double* rec_fac;      // [n] fac_max (1 right after a reject)
   int* rec_acc;         // [n]
   int* rec_rej;         // [n]
   int evict;            // 1: end-game eviction enabled
-  double big_steps;     // predicted remaining attempts above which an evicted reactor counts as a straggler
+  int cap;              // > 0: classification phase -- every reactor is handed on after `cap` attempts
+  double big_steps;     // predicted remaining attempts above which a reactor counts as a straggler (wide finisher)
+  // work list: null = reactors 0..n-1 from stats->queue; else resume reactors rlist[0 .. *rcount) (queue head *rqueue)
+  const int* rlist;
+  const unsigned long long* rcount;
+  unsigned long long* rqueue;
   double* V;  // [8][N][nslots]: 0 = y_n, 1..6 = f evaluations, 7 = stage argument
   DevStats* stats;
 };
@@ -93,19 +99,26 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
   if (tid == 0) s_qempty = 0;
   __syncthreads();
   unsigned long long lane_act = 0, lane_tot = 0, c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
+  const long long q_limit = a.rlist ? (long long)*a.rcount : a.n;
 
   // start an attempt from y_n: step-size guards of Algorithm 1, clip to t_f, stage argument = y_n
   auto begin_attempt = [&]() -> bool {
     if (nacc + nrej >= a.max_steps) { status = CK_ST_MAX_STEPS; return false; }
     if (!isfinite(h)) { status = CK_ST_NONFINITE; return false; }
     if (h < 1e-12 * a.dt) { status = CK_ST_H_UNDERFLOW; return false; }
-    if (endgame) {  // re-batch: hand this reactor to the cooperative finisher (state is at an attempt boundary)
+    const bool capped = a.cap > 0 && nacc + nrej >= a.cap;
+    if (endgame || capped) {  // re-batch: hand this reactor on (its state is at an attempt boundary)
       for (int c = 0; c < N; ++c) a.y[(size_t)c * a.ld + r] = Vy[c * ns];
       a.rec_t[r] = t; a.rec_h[r] = h; a.rec_fac[r] = fac_max; a.rec_acc[r] = nacc; a.rec_rej[r] = nrej;
-      // two classes: reactors whose predicted number of remaining attempts (t_f - t) / h is large go to the wide,
-      // latency-optimised finisher (one CTA per SM each), the mass to the throughput-oriented one
-      if ((a.dt - t) > a.big_steps * h) a.elist[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_b, 1ULL)] = (int)r;
-      else a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
+      if (capped) {
+        // classification: reactors whose predicted number of remaining attempts (t_f - t) / h is large are the critical
+        // chains of the batch -- they go to the wide, latency-optimised finisher AT ONCE (it runs beside the resumed
+        // thread-per-reactor phase of everybody else)
+        if ((a.dt - t) > a.big_steps * h) a.elist[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_b, 1ULL)] = (int)r;
+        else a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
+      } else {
+        a.elist2[atomicAdd(&a.stats->n_evicted_n, 1ULL)] = (int)r;   // end-game: the throughput-oriented finisher
+      }
       r = -1;
       return true;
     }
@@ -142,21 +155,27 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
     if (idle && (a.refill || idle == 0xffffffffu)) {
       const int cnt = a.refill ? __popc(idle) : 32;
       unsigned long long base = 0;
-      if (lane == 0) base = atomicAdd(&a.stats->queue, (unsigned long long)cnt);
+      if (lane == 0) base = atomicAdd(a.rqueue, (unsigned long long)cnt);
       base = __shfl_sync(0xffffffffu, base, 0);
       if (r < 0) {
         const long long cand = (long long)base + (a.refill ? __popc(idle & ((1u << lane) - 1)) : lane);
-        if (cand < a.n) {
-          r = cand;
+        if (cand < q_limit) {
+          r = a.rlist ? (long long)a.rlist[cand] : cand;
           p = a.p[r];
           for (int c = 0; c < N; ++c) {
             const double v = a.y[(size_t)c * a.ld + r];
             Vy[c * ns] = v;
             Vy[7 * vs + c * ns] = v;
           }
-          t = 0; nacc = 0; nrej = 0; status = CK_ST_OK; fac_max = 5.0; h_used = 0; last = false;
-          if (a.h0 > 0.0) { h = a.h0; if (!begin_attempt()) finish(); }
-          else st = ST_H0A;
+          status = CK_ST_OK; h_used = 0; last = false;
+          if (a.rlist) {  // resume from the hand-over record
+            t = a.rec_t[r]; h = a.rec_h[r]; fac_max = a.rec_fac[r]; nacc = a.rec_acc[r]; nrej = a.rec_rej[r];
+            if (!begin_attempt()) finish();
+          } else {
+            t = 0; nacc = 0; nrej = 0; fac_max = 5.0;
+            if (a.h0 > 0.0) { h = a.h0; if (!begin_attempt()) finish(); }
+            else st = ST_H0A;
+          }
         } else {
           s_qempty = 1;  // the queue ran dry (benign race: every writer stores 1)
         }
@@ -274,14 +293,16 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
     c.tptr = s_tptr; c.tent = s_tent;
     __syncthreads();
   }
-  const long long n_ev = (long long)(cls ? a.stats->n_evicted_b : a.stats->n_evicted);
+  WideRegs wr;
+  if constexpr (WIDE) wide_setup<G>(m, wr);
+  const long long n_ev = (long long)(cls ? a.stats->n_evicted_b : a.stats->n_evicted_n);
   unsigned long long c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
   for (;;) {
     __syncthreads();
     if (tid == 0) s_next = (long long)atomicAdd(cls ? &a.stats->queue_b : &a.stats->queue2, 1ULL);
     __syncthreads();
     if (s_next >= n_ev) break;
-    const long long r = a.elist[cls ? a.n - 1 - s_next : s_next];
+    const long long r = cls ? a.elist[a.n - 1 - s_next] : a.elist2[s_next];
     const double p = a.p[r];
     for (int i = tid; i < N; i += G) Y[i] = a.y[(size_t)i * a.ld + r];
     double t = a.rec_t[r], h = a.rec_h[r], fac_max = a.rec_fac[r], h_used = 0.0;
@@ -294,7 +315,7 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
       bool last = false;
       if (h >= a.dt - t) { h = a.dt - t; last = true; }
       TState ts;
-      if constexpr (WIDE) rhs_wide<G>(m, Y, p, F, c, ts);
+      if constexpr (WIDE) rhs_wide<G>(m, Y, p, F, c, ts, wr);
       else rhs_coop<G, false>(m, Y, p, F, c, ts);
       for (int s = 0; s < 5; ++s) {
         for (int i = tid; i < N; i += G) {
@@ -303,7 +324,7 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
           YT[i] = fma(h, acc, Y[i]);
         }
         __syncthreads();
-        if constexpr (WIDE) rhs_wide<G>(m, YT, p, F + (s + 1) * N, c, ts);
+        if constexpr (WIDE) rhs_wide<G>(m, YT, p, F + (s + 1) * N, c, ts, wr);
         else rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
       }
       c_rhs += 6;
@@ -401,16 +422,40 @@ int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
 inline size_t al256(size_t x) { return (x + 255) & ~size_t(255); }
 }  // namespace
 
-// workspace: [DevStats][int attempts[n]][hand-over records: 3 int + 3 double per reactor][double V[8][N][nslots]]
+namespace {
+// slots of the per-slot stage vectors: the plan for n reactors, with room for the plan of any smaller resumed batch
+inline size_t rkf_vslots(const RkfPlan& pl, int64_t n) { return std::max<size_t>((size_t)pl.grid * pl.block, (size_t)n + 512); }
+
+int32_t launch_main(const ck_mech* m, const RkfPlan& pl, const RkfArgs& a, long long grid, cudaStream_t st) {
+  switch (pl.block) {
+    case 512: rkf45_kernel<512, true><<<(unsigned)grid, 512, pl.smem, st>>>(m->dev, a); break;
+    case 256: rkf45_kernel<256, false><<<(unsigned)grid, 256, pl.smem, st>>>(m->dev, a); break;
+    case 128: rkf45_kernel<128, false><<<(unsigned)grid, 128, pl.smem, st>>>(m->dev, a); break;
+    case 64: rkf45_kernel<64, false><<<(unsigned)grid, 64, pl.smem, st>>>(m->dev, a); break;
+    default: rkf45_kernel<32, false><<<(unsigned)grid, 32, pl.smem, st>>>(m->dev, a); break;
+  }
+  CK_CUDA(cudaGetLastError());
+  return CK_OK;
+}
+}  // namespace
+
+// workspace: [DevStats][int attempts[n]][hand-over: 4 int + 3 double per reactor][double V[8][N][slots]]
 size_t ck_rkf_workspace(const ck_mech* m, int64_t n) {
   if (n == 0) return sizeof(DevStats);
   RkfPlan pl;
   if (rkf_plan(m, n, &pl) != CK_OK) return sizeof(DevStats);  // the integrate call reports the error
-  const size_t nslots = (size_t)pl.grid * pl.block;
-  return sizeof(DevStats) + 4 * al256((size_t)n * sizeof(int)) + 3 * al256((size_t)n * sizeof(double)) +
-         (size_t)8 * (m->K + 1) * nslots * sizeof(double);
+  return sizeof(DevStats) + 5 * al256((size_t)n * sizeof(int)) + 3 * al256((size_t)n * sizeof(double)) +
+         (size_t)8 * (m->K + 1) * rkf_vslots(pl, n) * sizeof(double);
 }
 
+// Flow (flags = 0, models with N > 32):
+//   1  classification: the thread-per-reactor kernel over all reactors, every reactor handed on after RKF_CAP attempts
+//      (most of config 4's reactors need more); predicted stragglers -> list W, the others -> list C
+//   2a the wide finisher over list W on a SECOND stream, one 384-thread CTA per straggler (their serial chains are the
+//      critical path, so they start now and run beside 2b / 3)
+//   2b the thread-per-reactor kernel resumes list C (lane refill; end-game eviction -> list N)
+//   3  the narrow finisher over list N (64 / 128-thread CTAs, many per SM)
+// N <= 32: phases 1 (uncapped, with end-game eviction) and 3 only.  flags bit 0 / 1: one kernel, no eviction.
 extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt,
                                       const ck_opts* o, int32_t* n_accept, int32_t* n_reject, int32_t* status,
                                       double* h_last, void* ws, size_t ws_bytes, ck_report* report, void* stream) {
@@ -418,13 +463,14 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   if (!m) { set_error("ck_integrate_rkf45: null mechanism"); return CK_EINVAL; }
   RkfPlan pl;
   if (n > 0) { int32_t rc0 = rkf_plan(m, n, &pl); if (rc0) return rc0; }
-  const size_t nslots = (size_t)pl.grid * pl.block;
+  const size_t nslots = n > 0 ? rkf_vslots(pl, n) : 0;
   const size_t bi = al256((size_t)n * sizeof(int)), bd = al256((size_t)n * sizeof(double));
-  const size_t need = n > 0 ? sizeof(DevStats) + 4 * bi + 3 * bd + (size_t)8 * (m->K + 1) * nslots * sizeof(double) : sizeof(DevStats);
+  const size_t need = n > 0 ? sizeof(DevStats) + 5 * bi + 3 * bd + (size_t)8 * (m->K + 1) * nslots * sizeof(double) : sizeof(DevStats);
   int32_t rc = integrate_prologue("ck_integrate_rkf45", m, n, y, ld, p, dt, o, ws, ws_bytes, need, st);
   if (rc) return rc;
   if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
-  RkfArgs a;
+  const int N = m->K + 1;
+  RkfArgs a{};
   a.n = n; a.ld = ld; a.nslots = (long long)nslots; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
   a.max_steps = o->max_steps > 0 ? o->max_steps : 100000; a.refill = !(o->flags & 1);
   a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
@@ -432,47 +478,81 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   char* wp = (char*)ws + sizeof(DevStats);
   a.att = (int*)wp; wp += bi;
   a.elist = (int*)wp; wp += bi;
+  a.elist2 = (int*)wp; wp += bi;
   a.rec_acc = (int*)wp; wp += bi;
   a.rec_rej = (int*)wp; wp += bi;
   a.rec_t = (double*)wp; wp += bd;
   a.rec_h = (double*)wp; wp += bd;
   a.rec_fac = (double*)wp; wp += bd;
   a.V = (double*)wp;
-  a.evict = (o->flags & 3) ? 0 : 1;  // bit 0: static mapping, bit 1: refill only (no finisher)
-  a.big_steps = (m->K + 1 > 32) ? 2000.0 : 1e300;
-  switch (pl.block) {
-    case 512: rkf45_kernel<512, true><<<(unsigned)pl.grid, 512, pl.smem, st>>>(m->dev, a); break;
-    case 256: rkf45_kernel<256, false><<<(unsigned)pl.grid, 256, pl.smem, st>>>(m->dev, a); break;
-    case 128: rkf45_kernel<128, false><<<(unsigned)pl.grid, 128, pl.smem, st>>>(m->dev, a); break;
-    case 64: rkf45_kernel<64, false><<<(unsigned)pl.grid, 64, pl.smem, st>>>(m->dev, a); break;
-    default: rkf45_kernel<32, false><<<(unsigned)pl.grid, 32, pl.smem, st>>>(m->dev, a); break;
-  }
-  CK_CUDA(cudaGetLastError());
+  const bool finishers = !(o->flags & 3);          // bit 0: static mapping, bit 1: refill only (no finisher)
+  const bool classify = finishers && N > 32;
+  constexpr int RKF_CAP = 24;                       // attempts before a reactor is classified
+  constexpr double RKF_BIG = 12000.0;               // predicted remaining attempts that make a straggler
+  a.rlist = nullptr; a.rcount = nullptr; a.rqueue = &a.stats->queue;
+  a.cap = classify ? std::min(RKF_CAP, a.max_steps) : 0;
+  a.big_steps = RKF_BIG;
+  a.evict = (finishers && !classify) ? 1 : 0;
+  // everything the finishers need is validated BEFORE the first launch: a failure must not leave y half-integrated
+  const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R, m->dev.n_tent) * sizeof(double);
+  if (finishers && smem2 > 227 * 1024) { set_error("ck_integrate_rkf45: mechanism too large for the cooperative finisher"); return CK_EUNSUPPORTED; }
+  int sms = 0;
+  CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  rc = launch_main(m, pl, a, pl.grid, st);
+  if (rc) return rc;
   int rounds = 1;
-  if (a.evict) {  // finisher over the eviction list (its length is read on the device)
-    const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R, m->dev.n_tent) * sizeof(double);
-    if (smem2 > 227 * 1024) { set_error("ck_integrate_rkf45: mechanism too large for the cooperative finisher"); return CK_EUNSUPPORTED; }
-    int per_sm = 0, sms = 0;
-    const int N = m->K + 1;
-    CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
-    // threads per evicted reactor: the finisher runs the stragglers' serial chains, so its time is the latency of one
-    // cooperative RHS x 6 x the attempts of the slowest reactor; wider CTAs shorten the reaction loop of that RHS
-    const long long cap = (long long)n;
-    auto launch_fin = [&](auto kern, int G, int cls) -> int32_t {
+  if (finishers) {
+    int per_sm = 0;
+    auto launch_fin = [&](auto kern, int G, int cls, long long want, cudaStream_t s) -> int32_t {
       CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
       CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G, smem2));
-      kern<<<(unsigned)std::min<long long>(cap, (long long)std::max(per_sm, 1) * sms), G, smem2, st>>>(m->dev, a, cls);
+      const long long grid = std::max<long long>(1, std::min<long long>(want, (long long)std::max(per_sm, 1) * sms));
+      kern<<<(unsigned)grid, G, smem2, s>>>(m->dev, a, cls);
+      CK_CUDA(cudaGetLastError());
       return CK_OK;
     };
-    // the mass of the evicted reactors: many narrow CTAs per SM (throughput); the predicted stragglers: one wide CTA each
-    int32_t rcf;
-    if (N <= 32) rcf = launch_fin(rkf45_coop_kernel<32, false>, 32, 0);
-    else if (N <= 64) rcf = launch_fin(rkf45_coop_kernel<64, false>, 64, 0);
-    else rcf = launch_fin(rkf45_coop_kernel<128, false>, 128, 0);
-    if (rcf) return rcf;
-    if (N > 32) { rcf = launch_fin(rkf45_coop_kernel<384, true>, 384, 1); if (rcf) return rcf; }
-    CK_CUDA(cudaGetLastError());
-    rounds = (N > 32) ? 3 : 2;
+    cudaStream_t s2 = nullptr;
+    cudaEvent_t ev_fin = nullptr;
+    if (classify) {
+      DevStats hs;   // the two list lengths size the next launches (one small read-back; this call synchronises anyway)
+      CK_CUDA(cudaMemcpyAsync(&hs, a.stats, sizeof hs, cudaMemcpyDeviceToHost, st));
+      CK_CUDA(cudaStreamSynchronize(st));
+      const long long nW = (long long)hs.n_evicted_b, nC = (long long)hs.n_evicted;
+      if (nW > 0) {   // 2a: the stragglers, beside everything that follows
+        cudaEvent_t ev_main = nullptr;
+        CK_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+        CK_CUDA(cudaEventCreateWithFlags(&ev_main, cudaEventDisableTiming));
+        CK_CUDA(cudaEventCreateWithFlags(&ev_fin, cudaEventDisableTiming));
+        CK_CUDA(cudaEventRecord(ev_main, st));
+        CK_CUDA(cudaStreamWaitEvent(s2, ev_main, 0));
+        rc = launch_fin(rkf45_coop_kernel<384, true>, 384, 1, nW, s2);
+        cudaEventDestroy(ev_main);
+        if (rc) return rc;
+        CK_CUDA(cudaEventRecord(ev_fin, s2));
+        rounds++;
+      }
+      if (nC > 0) {   // 2b: resume the rest thread-per-reactor
+        RkfPlan pl2;
+        rc = rkf_plan(m, nC, &pl2);
+        if (rc) return rc;
+        a.cap = 0; a.evict = 1;
+        a.rlist = a.elist; a.rcount = &a.stats->n_evicted; a.rqueue = &a.stats->queue_c;
+        rc = launch_main(m, pl2, a, pl2.grid, st);
+        if (rc) return rc;
+        rounds++;
+      }
+    }
+    // 3: whatever the end-game evicted (its count is read on the device)
+    if (N <= 32) rc = launch_fin(rkf45_coop_kernel<32, false>, 32, 0, n, st);
+    else if (N <= 64) rc = launch_fin(rkf45_coop_kernel<64, false>, 64, 0, n, st);
+    else rc = launch_fin(rkf45_coop_kernel<128, false>, 128, 0, n, st);
+    if (rc) return rc;
+    rounds++;
+    if (s2) {   // join the second stream; both objects are released once their work has drained
+      CK_CUDA(cudaStreamWaitEvent(st, ev_fin, 0));
+      cudaEventDestroy(ev_fin);
+      cudaStreamDestroy(s2);
+    }
   }
   return integrate_report(m, n, a.att, a.stats, rounds, 0, report, st);
 }

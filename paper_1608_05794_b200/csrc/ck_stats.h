@@ -12,7 +12,7 @@ struct DevStats {
   unsigned long long attempts, accepted, rejected, rhs_evals, jac_evals, failed;
   unsigned long long lane_active;  // lane-slots that did useful work in the step-attempt loop
   unsigned long long lane_total;   // lane-slots issued
-  unsigned long long n_evicted;    // reactors handed from the thread-per-reactor phase to the cooperative finisher
+  unsigned long long n_evicted;    // reactors the capped classification phase hands on to the resumed thread-per-reactor phase
   unsigned long long queue2;       // work-queue head of the finisher
   unsigned long long qempty;       // set once the main queue ran dry
   unsigned long long clk[8];       // ROS4 phase clocks (SM cycles summed over CTAs): 0 RHS+dq, 1 Jacobian assembly,
@@ -20,7 +20,9 @@ struct DevStats {
   unsigned long long n_evicted_b;  // ... of which predicted stragglers (handed to the wide low-latency finisher; listed from
                                    // the back of the eviction list)
   unsigned long long queue_b;      // work-queue head of the wide finisher
-  unsigned long long pad[10];
+  unsigned long long n_evicted_n;  // reactors handed to the narrow (throughput) finisher at the end-game
+  unsigned long long queue_c;      // work-queue head of the resumed thread-per-reactor phase
+  unsigned long long pad[8];
 };
 static_assert(sizeof(DevStats) == 256, "DevStats is the 256-byte header of the workspace");
 

@@ -153,7 +153,7 @@ def test_rkf45_static_vs_refill(oracle):
     assert r2["report"]["simt_efficiency"] >= r1["report"]["simt_efficiency"] - 1e-9
     g3, r3, ref3, _ = _run(oracle, "C4", 2048, flags=0)      # refill + cooperative finisher for the stragglers
     _check(g3, r3, ref3, 53, tight=ref3["tight"])
-    assert r3["report"]["rounds"] == 3
+    assert r3["report"]["rounds"] >= 3
     # Eq. 20 at P = 32 from the attempt counts equals 1 - efficiency of the static mapping up to tail effects
     assert r1["report"]["waste_p32"] > 0
 
