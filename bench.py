@@ -31,8 +31,8 @@ UNIT = "RHS evals/s"
 # 148 SMs x 64 FP64 FMA lanes/clk x 1.965 GHz = 1.861e13 FP64-pipe instructions ("slots")/s = 37.2 TFLOP/s
 PEAK_SLOTS = 148 * 64 * 1.965e9
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE rhs_kernel_tmem<512> launch over the full 1,048,576 states
-# (ncu --set full, profiles/r02_rhs_kernel_full.md); None until such a capture of the full-size launch exists
-RHS_DRAM_BYTES_PER_LAUNCH_FULL = 865.98e6
+# (ncu --set full, profiles/r02_kernels.md); None until such a capture of the full-size launch exists
+RHS_DRAM_BYTES_PER_LAUNCH_FULL = 869.1e6
 
 
 def measured_hbm_gbs():
@@ -295,6 +295,25 @@ def run_case(args):
     import paper_1608_05794_b200 as ck
     from synth_inputs import make_config
     dev = torch.device("cuda", 0)
+    if args.case == "lu":   # the dense linear algebra on its own: ck_lu_solve_batched (warp-per-system blocked LU, DMMA trailing update)
+        out = {"case": "lu", "dfma_peak_per_s": ck.fp64_peak(0), "dmma_peak_fma_per_s": ck.fp64_mma_peak(0)}
+        for N, n in ((54, 65536), (112, 16384), (15, 262144)):
+            g = torch.Generator(device="cuda").manual_seed(7)
+            A = torch.rand((n, N, N), dtype=torch.float64, device=dev, generator=g) - 0.5 + 4.0 * torch.eye(N, dtype=torch.float64, device=dev)
+            b = torch.rand((n, N), dtype=torch.float64, device=dev, generator=g)
+            ck.lu_solve_batched(A, b)
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                ck.lu_solve_batched(A, b)
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 5
+            fma = N ** 3 / 3.0 + N * N
+            out[f"N{N}"] = {"systems": n, "ms": ms, "systems_per_s": n / (ms * 1e-3), "fma_per_system": fma,
+                            "frac_of_fp64_peak": fma * n / (ms * 1e-3) / PEAK_SLOTS,
+                            "hbm_GBs": (N * N + 2 * N) * 8 * n / (ms * 1e-3) / 1e9}
+        print(json.dumps(out))
+        return
     name = "C2" if args.case == "rhs" else args.case
     mech, y, p, cfg = make_config(name)
     M = ck.Mechanism(mech, device=0)
@@ -379,9 +398,10 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     achieved = slots * n / (per_launch_ms * 1e-3)
-    measured_peak = None
+    measured_peak = mma_peak = None
     try:
         measured_peak = ck.fp64_peak(local)
+        mma_peak = ck.fp64_mma_peak(local)
     except Exception:
         pass
     traffic = RHS_DRAM_BYTES_PER_LAUNCH_FULL if n == 1048576 else None
@@ -390,7 +410,7 @@ def run_ours(args):
                 "unit": "TFLOP/s", "frac": achieved / PEAK_SLOTS, "traffic": traffic,
                 "peak_source": "derived and probed FP64 peak (MEASURED_PEAKS.json carries no FP64 figure): 148 SM x 64 FP64 FMA/clk x 1.965 GHz (DESIGN.md); 1 FP64-pipe instruction = 2 flop",
                 "slots_per_eval": slots, "fp64_pipe_inst_per_s": achieved,
-                "measured_dfma_peak_inst_per_s": measured_peak,
+                "measured_dfma_peak_inst_per_s": measured_peak, "measured_dmma_peak_fma_per_s": mma_peak,
                 "frac_of_measured_dfma_peak": (achieved / measured_peak) if measured_peak else None,
                 "hbm_alg_bytes_per_launch": alg_bytes, "hbm_achieved_GBs": alg_bytes / (per_launch_ms * 1e-3) / 1e9,
                 "hbm_peak_GBs": hbm_gbs, "hbm_peak_source": hbm_src,

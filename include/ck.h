@@ -189,6 +189,9 @@ int32_t ck_rhs_slots(const ck_mech* m, double* slots);
 int32_t ck_rhs_variant(const ck_mech* m, int64_t n, int32_t* block, int32_t* tmem);
 /* Measure the FP64 FMA peak of the device with a register-resident DFMA chain (slots/s). */
 int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream);
+/* The same through the FP64 tensor cores (mma.sync.m8n8k4.f64, 256 FMA per warp instruction): FMA/s.  On B200 it equals
+ * the vector rate (64 FMA/clk/SM), so DMMA buys instruction count and operand traffic, not flops. */
+int32_t ck_fp64_mma_peak(int32_t device, double* fma_per_s, void* stream);
 
 /* Waste of each SIMD work unit, Eq. 20: W_j = 1 - sum_i N_i / (P max_i N_i) over the P
  * consecutive reactors of unit j under the static linear reactor -> lane mapping, N_i = attempts of

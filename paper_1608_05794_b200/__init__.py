@@ -4,5 +4,5 @@ Thin binding over the C-ABI library libck.so (include/ck.h): argument marshallin
 the path runs in the library's CUDA kernels.  There is no CPU fallback: importing works without a GPU
 (so the ABI can be inspected), but any compute call without the library or a device raises.
 """
-from ._binding import (Mechanism, CkError, lib, lib_path, exported_symbols, fp64_peak, lu_solve_batched, parse_mechanism,  # noqa: F401
+from ._binding import (Mechanism, CkError, lib, lib_path, exported_symbols, fp64_peak, fp64_mma_peak, lu_solve_batched, parse_mechanism,  # noqa: F401
                        CK_OP_ROS, CK_OP_RKF45, CK_OP_JAC, CK_JAC_ANALYTIC, CK_JAC_FD)

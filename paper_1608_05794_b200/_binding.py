@@ -64,7 +64,7 @@ def lib():
         L.ck_last_error.restype = C.c_char_p
         for name in ("ck_mech_load", "ck_mech_free", "ck_mech_sizes", "ck_mech_set_reactor", "ck_workspace_bytes", "ck_rhs", "ck_jac",
                      "ck_integrate_ros", "ck_integrate_rkf45", "ck_rhs_host", "ck_integrate_host", "ck_rhs_slots",
-                     "ck_fp64_peak", "ck_version", "ck_jac_batched", "ck_jac_batched_static", "ck_jac_static_max_reactors", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks", "ck_mech_parse", "ck_parsed_name",
+                     "ck_fp64_peak", "ck_fp64_mma_peak", "ck_version", "ck_jac_batched", "ck_jac_batched_static", "ck_jac_static_max_reactors", "ck_lu_solve_batched", "ck_rhs_variant", "ck_waste", "ck_waste_tasks", "ck_mech_parse", "ck_parsed_name",
                      "ck_parsed_free"):
             getattr(L, name).restype = C.c_int32
         L.ck_parsed_desc.restype = C.POINTER(MechDesc)
@@ -154,6 +154,12 @@ def lu_solve_batched(A, b):
     x = torch.empty_like(b); st = torch.zeros(n, dtype=torch.int32, device=A.device)
     _check(lib().ck_lu_solve_batched(int(N), C.c_int64(n), _ptr(A), _ptr(b), _ptr(x), _ptr(st), _stream()))
     return x, st
+
+
+def fp64_mma_peak(device=0):
+    v = C.c_double(0)
+    _check(lib().ck_fp64_mma_peak(int(device), C.byref(v), None))
+    return v.value
 
 
 class Mechanism:

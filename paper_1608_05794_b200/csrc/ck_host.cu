@@ -30,7 +30,51 @@ __global__ void __launch_bounds__(256) dfma_probe(double* out, double a, double 
   out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+// the same for the FP64 tensor-core path: 8 independent m8n8k4 accumulator tiles per warp (256 FMA per instruction)
+__global__ void __launch_bounds__(256) dmma_probe(double* out, double a, double b, int iters) {
+  double c[8][2];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) { c[i][0] = threadIdx.x + i; c[i][1] = i; }
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[i][0]), "+d"(c[i][1]) : "d"(a), "d"(b));
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += c[i][0] + c[i][1];
+  out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace
+
+extern "C" int32_t ck_fp64_mma_peak(int32_t device, double* fma_per_s, void* stream) {
+  if (!fma_per_s) { set_error("ck_fp64_mma_peak: null output"); return CK_EINVAL; }
+  CK_CUDA(cudaSetDevice(device));
+  cudaStream_t st = (cudaStream_t)stream;
+  int sms = 0;
+  CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+  const int blocks = sms * 4, threads = 256, iters = 8192;
+  double* out = nullptr;
+  CK_CUDA(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));
+  cudaEvent_t e0, e1;
+  CK_CUDA(cudaEventCreate(&e0));
+  CK_CUDA(cudaEventCreate(&e1));
+  double best = 0;
+  for (int rep = 0; rep < 6; ++rep) {
+    CK_CUDA(cudaEventRecord(e0, st));
+    dmma_probe<<<blocks, threads, 0, st>>>(out, 1.0000001, 0.9999999, iters);
+    CK_CUDA(cudaEventRecord(e1, st));
+    CK_CUDA(cudaEventSynchronize(e1));
+    float ms = 0;
+    CK_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    const double rate = (double)blocks * (threads / 32) * iters * 8.0 * 256.0 / (ms * 1e-3);
+    if (rep >= 1) best = std::max(best, rate);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+  *fma_per_s = best;
+  return CK_OK;
+}
 
 extern "C" int32_t ck_fp64_peak(int32_t device, double* dfma_per_s, void* stream) {
   if (!dfma_per_s) { set_error("ck_fp64_peak: null output"); return CK_EINVAL; }
