@@ -41,20 +41,25 @@ static int32_t launch_rhs(const ck_mech* m, long long n, const double* y, long l
 // accumulators in tensor memory: BLOCK threads per CTA, persistent over batches of BLOCK reactors.  512 threads (one
 // CTA per SM) for large batches of models with K + 1 <= 64; 128 threads (up to three CTAs per SM) when the batch
 // would leave most SMs without a 512-thread CTA; 224 threads (seven warps, two column sets) for 64 < K + 1 <= 124.
-template <int BLOCK>
-static int32_t launch_rhs_tmem(const ck_mech* m, long long n, const double* y, long long ld, const double* p, double* f,
-                               long long ldf, cudaStream_t st) {
+template <int BLOCK, int CVM>
+static int32_t launch_rhs_tmem_kind(const ck_mech* m, long long n, const double* y, long long ld, const double* p, double* f,
+                                    long long ldf, cudaStream_t st) {
   const size_t smem = rhs_tmem_smem_bytes(m->K, m->dev.rstride, BLOCK);
-  CK_CUDA(cudaFuncSetAttribute(rhs_kernel_tmem<BLOCK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CK_CUDA(cudaFuncSetAttribute(rhs_kernel_tmem<BLOCK, CVM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int sms = 0;
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
   const int cols = rhs_tmem_cols(m->K, BLOCK);
   const long long per_sm = std::max<long long>(1, std::min<long long>(512 / cols, (long long)((227 * 1024) / (smem + 1024))));
   const long long batches = (n + BLOCK - 1) / BLOCK;
   const long long grid = std::min<long long>(batches, per_sm * sms);
-  rhs_kernel_tmem<BLOCK><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, n, y, ld, p, f, ldf);
+  rhs_kernel_tmem<BLOCK, CVM><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, n, y, ld, p, f, ldf);
   CK_CUDA(cudaGetLastError());
   return CK_OK;
+}
+template <int BLOCK>
+static int32_t launch_rhs_tmem(const ck_mech* m, long long n, const double* y, long long ld, const double* p, double* f,
+                               long long ldf, cudaStream_t st) {
+  return m->dev.cv ? launch_rhs_tmem_kind<BLOCK, 1>(m, n, y, ld, p, f, ldf, st) : launch_rhs_tmem_kind<BLOCK, 0>(m, n, y, ld, p, f, ldf, st);
 }
 
 // CTA width of the tensor-memory kernel for this batch; 0: use the shared-memory kernel
