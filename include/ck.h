@@ -143,7 +143,8 @@ int32_t ck_jac_batched(const ck_mech* m, int64_t n, const double* y, int64_t ld,
 
 /* ck_jac_batched for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid
  * cudaMalloc): same kernels, same output, but the scratch lives in a file-scope device array of CK_JAC_STATIC_BYTES that
- * every GPU loading the library holds until exit -- no workspace argument, no cudaMalloc / cudaFree inside.
+ * every GPU loading the library holds until exit (the driver maps it with the module, lazily: on the first use of this
+ * entry point on that device) -- no workspace argument, no cudaMalloc / cudaFree inside.
  * CK_EWORKSPACE (with the limit in ck_last_error()) when n reactors of this model need more scratch than that;
  * ck_jac_static_max_reactors gives the largest n that fits (2,761 for a 53-species / 325-reaction model, 1,161 for
  * 111 / 784).  All calls on one device share the array, which keeps the last call's contents (nothing needs clearing:
