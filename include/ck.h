@@ -74,7 +74,9 @@ typedef struct {
   double h0;
   int32_t max_steps;
   int32_t flags;       /* bit 0: disable the divergence-control layer (static reactor -> lane / CTA mapping, the paper's
-                          layout; for comparison).  RKF45, bit 1: lane refill only, no cooperative finisher.
+                          layout; for comparison).  RKF45, bit 1: lane refill only, no cooperative finisher; bits 4 / 5
+                          (measurement of the finishers): every reactor counts as a straggler after the classification
+                          pass / the stragglers run on the narrow finisher instead of the wide one.
                           ROS4, bit 2: force the fused CTA-per-reactor kernel, bit 3: force the batched rounds
                           (default: rounds for n >= 16384 reactors of a model with 33 <= N <= 128, analytic Jacobian). */
 } ck_opts;

@@ -60,8 +60,6 @@ struct CoopChem {
   double* tau;   // [K]    sum_i nu_ki dq_i/dT|_C
   int* dsl;      // [6][R] slot species of every reaction (shared-memory copy: the row assembly would otherwise
                  //        wait on a global load per reaction)
-  const int* tptr;  // transposed stoichiometry for the production-rate gather of rhs_wide: shared-memory copies when
-  const int* tent;  //        the caller staged them (rkf45_coop_kernel), else the global arrays
 };
 struct CoopScalars { double rho, S, cps, Ctot, hw; };
 
@@ -88,7 +86,6 @@ __device__ __forceinline__ CoopChem coop_carve(double* base, int K, int R, bool 
   c.sig = base; base += jac ? K : 0;
   c.tau = base; base += jac ? K : 0;
   c.dsl = reinterpret_cast<int*>(base);
-  c.tptr = nullptr; c.tent = nullptr;
   return c;
 }
 
@@ -168,139 +165,6 @@ __device__ __forceinline__ CoopScalars rhs_coop(const MechDev& m, const double* 
   if (tid == 0) fout[0] = -(t.T * s.hw) / (s.rho * s.cps);
   __syncthreads();
   return s;
-}
-
-// f = RHS(y; p) with a WIDE CTA (G >= 4 warps, ideally G >= R): the latency-optimised evaluation for the serial step
-// chains of the RKF45 stragglers (ck_rkf.cu).  Species k is thread k (thermo, concentration), reaction r is thread r (a
-// single trip when G >= R), QS adjacent lanes share one species row in the production-rate gather, whose entries sit in
-// registers (WideRegs).  Every thread takes ln T and 1 / T itself, the reductions run only in the warps that hold data,
-// and the divisions on the critical path (rho, 1 / rho, T-dot) use the few-ulp reciprocal ck_rcp.  Measured on the
-// 53 / 325 model (one CTA alone on an SM): 6.6 k cycles per evaluation, of which 2.9 k waiting for the Troe rows
-// (single-warp chains of five exponentials and two logarithms); moving their T-only part into the thermo phase was
-// measured and did not shorten the evaluation (the critical thread moves with it).  Ends with a __syncthreads().
-// Per-thread, per-kernel-lifetime registers of rhs_wide: the (reaction, nu) entries of this thread's share of its species
-// row of the transposed stoichiometry, and the species' molar mass.  Loaded once (wide_setup); the evaluation then
-// gathers with independent shared-memory loads of q instead of a chain tptr -> tent -> q per entry.
-constexpr int WIDE_MAXE = 12;
-struct WideRegs {
-  int ent[WIDE_MAXE];   // (reaction << 8) | (nu + 128)
-  int ne;               // entries in use; -1: the row does not fit, walk the lists instead
-  double Wk;
-};
-template <int G>
-__device__ __forceinline__ void wide_setup(const MechDev& m, WideRegs& wr) {
-  const int K = m.K, tid = threadIdx.x;
-  const int QS = (4 * K <= G) ? 4 : ((2 * K <= G) ? 2 : 1);
-  const int k = tid / QS, part = tid % QS;
-  wr.ne = 0; wr.Wk = 0.0;
-#pragma unroll
-  for (int e = 0; e < WIDE_MAXE; ++e) wr.ent[e] = 128;
-  bool fits = true;
-  for (int kk = 0; kk < K; ++kk) fits = fits && (__ldg(m.tptr + kk + 1) - __ldg(m.tptr + kk) <= QS * WIDE_MAXE);
-  if (!fits) { wr.ne = -1; if (k < K) wr.Wk = __ldg(m.W + k); return; }
-  if (k < K) {
-    wr.Wk = __ldg(m.W + k);
-    const int e1 = __ldg(m.tptr + k + 1);
-    int n = 0;
-#pragma unroll
-    for (int x = 0; x < WIDE_MAXE; ++x) {
-      const int e = __ldg(m.tptr + k) + part + x * QS;
-      if (e < e1) { wr.ent[x] = __ldg(m.tent + e); n = x + 1; }
-    }
-    wr.ne = n;
-  }
-}
-
-template <int G>
-__device__ __forceinline__ void rhs_wide(const MechDev& m, const double* __restrict__ y, double p, double* __restrict__ fout,
-                                         const CoopChem& c, TState& t, const WideRegs& wr) {
-  const int K = m.K, R = m.R, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KW = (K + 31) >> 5;          // warps holding species in the thermo phase
-  t = make_tstate(m, y[0]);              // every thread: ln T, 1 / T, temperature interval
-  const double T = t.T;
-  // ---- phase 1: species threads -> thermo sums; reaction threads -> everything that depends on T only -------------
-  double yw = 0.0, cp = 0.0;
-  if (warp < KW) {
-    if (tid < K) {
-      double cpR, hRT;
-      thermo_cp_h(m, tid, t, cpR, hRT);
-      const double sub = m.cv ? 1.0 : 0.0;   // constant volume: c_v,k and u_k (see rhs_coop)
-      yw = y[1 + tid] * __ldg(m.invW + tid);
-      c.hRT[tid] = hRT - sub;
-      cp = yw * (cpR - sub);
-    }
-    double S = yw;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { S += __shfl_xor_sync(0xffffffffu, S, o); cp += __shfl_xor_sync(0xffffffffu, cp, o); }
-    if (lane == 0) { c.red[warp] = S; c.red[8 + warp] = cp; }
-  }
-  __syncthreads();
-  // ---- phase 2: concentrations ------------------------------------------------------------------------------------
-  double S = 0.0, cps = 0.0;
-  for (int w = 0; w < KW; ++w) { S += c.red[w]; cps += c.red[8 + w]; }
-  const double rho = m.cv ? p : (p * t.invT * (1.0 / R_U)) * ck_rcp(S);
-  const double Ctot = m.cv ? rho * S : p * t.invT * (1.0 / R_U);
-  if (tid < K) c.C[tid] = rho * yw;
-  if (tid == 0) c.C[K] = 1.0;
-  __syncthreads();
-  // ---- phase 3: what is left of the rates of progress ---------------------------------------------------------------
-  for (int r = tid; r < R; r += G) {
-    const RxnConst kc = load_rxn_global(m, r, t.tint);
-    c.q[r] = reaction_q<1, false>(m, r, kc, t, c.C, Ctot, nullptr);
-  }
-  __syncthreads();
-  // ---- phase 4: production rates (QS adjacent lanes share one species row of the transposed stoichiometry) ----------
-  const int QS = (4 * K <= G) ? 4 : ((2 * K <= G) ? 2 : 1);
-  const int GW = (K * QS + 31) >> 5;     // warps holding species in the gather phase
-  const double irho = ck_rcp(rho);
-  if (warp < GW) {
-    const int k = tid / QS, part = tid % QS;
-    const int* tptr = c.tptr ? c.tptr : m.tptr;
-    const int* tent = c.tent ? c.tent : m.tent;
-    double w = 0.0;
-    if (wr.ne >= 0) {  // entries in registers: independent loads of q, three accumulation chains
-      double qv[WIDE_MAXE];
-#pragma unroll
-      for (int x = 0; x < WIDE_MAXE; ++x) qv[x] = (x < wr.ne) ? c.q[wr.ent[x] >> 8] : 0.0;
-      double w1 = 0.0, w2 = 0.0;
-#pragma unroll
-      for (int x = 0; x < WIDE_MAXE; x += 3) {
-        w = fma((double)((wr.ent[x] & 255) - 128), qv[x], w);
-        if (x + 1 < WIDE_MAXE) w1 = fma((double)((wr.ent[x + 1] & 255) - 128), qv[x + 1], w1);
-        if (x + 2 < WIDE_MAXE) w2 = fma((double)((wr.ent[x + 2] & 255) - 128), qv[x + 2], w2);
-      }
-      w += w1 + w2;
-    } else if (k < K) {
-      int e = tptr[k] + part;
-      const int e1 = tptr[k + 1];
-      double w1 = 0.0;
-      for (; e + QS < e1; e += 2 * QS) {   // two independent chains
-        const int en0 = tent[e], en1 = tent[e + QS];
-        w = fma((double)((en0 & 255) - 128), c.q[en0 >> 8], w);
-        w1 = fma((double)((en1 & 255) - 128), c.q[en1 >> 8], w1);
-      }
-      if (e < e1) { const int en0 = tent[e]; w = fma((double)((en0 & 255) - 128), c.q[en0 >> 8], w); }
-      w += w1;
-    }
-    if (QS >= 2) w += __shfl_xor_sync(0xffffffffu, w, 1);
-    if (QS >= 4) w += __shfl_xor_sync(0xffffffffu, w, 2);
-    double hwp = 0.0;
-    if (k < K && part == 0) {
-      hwp = c.hRT[k] * w;
-      fout[1 + k] = w * wr.Wk * irho;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) hwp += __shfl_xor_sync(0xffffffffu, hwp, o);
-    if (lane == 0) c.red[16 + warp] = hwp;
-  }
-  __syncthreads();
-  // ---- phase 5: the temperature equation ------------------------------------------------------------------------------
-  if (tid == 0) {
-    double hw = 0.0;
-    for (int w = 0; w < GW; ++w) hw += c.red[16 + w];
-    fout[0] = -(T * hw) * irho * ck_rcp(cps);
-  }
-  __syncthreads();
 }
 
 // f(y) AND the species rows G_kj of the analytic Jacobian in one pass over the reactions, G reactions at a time:

@@ -44,7 +44,8 @@ struct RkfArgs {
   int* att;
   // hand-over records of reactors evicted at an attempt boundary (finished by rkf45_coop_kernel)
   int* elist;           // [n] after the classification phase: reactors to resume (from the front), stragglers (from the back)
-  int* elist2;          // [n] reactors evicted at the end-game (narrow finisher)
+  int* elist2;          // [n] reactors evicted at the end-game (narrow finisher, from the front); middle class (from the back)
+  int* tmp;             // [n] scratch of rkf_bucket_kernel
   double* rec_t;        // [n] time reached
   double* rec_h;        // [n] next step size
   double* rec_fac;      // [n] fac_max (1 right after a reject)
@@ -53,6 +54,7 @@ struct RkfArgs {
   int evict;            // 1: end-game eviction enabled
   int cap;              // > 0: classification phase -- every reactor is handed on after `cap` attempts
   double big_steps;     // predicted remaining attempts above which a reactor counts as a straggler (wide finisher)
+  double mid_steps;     // ... above which it goes to the narrow finisher at once instead of being resumed thread-per-reactor
   // work list: null = reactors 0..n-1 from stats->queue; else resume reactors rlist[0 .. *rcount) (queue head *rqueue)
   const int* rlist;
   const unsigned long long* rcount;
@@ -60,6 +62,69 @@ struct RkfArgs {
   double* V;  // [8][N][nslots]: 0 = y_n, 1..6 = f evaluations, 7 = stage argument
   DevStats* stats;
 };
+
+// Finisher work lists: cls 0 = end-game evictions (front of elist2), 1 = stragglers (back of elist), 2 = middle class
+// (back of elist2).  Lists 1 and 2 may be re-ordered longest-first by rkf_order_kernel before they are consumed.
+__device__ __forceinline__ long long fin_count(const RkfArgs& a, int cls) {
+  return (long long)(cls == 1 ? a.stats->n_evicted_b : (cls == 2 ? a.stats->n_evicted_m : a.stats->n_evicted_n));
+}
+__device__ __forceinline__ unsigned long long* fin_queue(const RkfArgs& a, int cls) {
+  return cls == 1 ? &a.stats->queue_b : (cls == 2 ? &a.stats->queue_m : &a.stats->queue2);
+}
+__device__ __forceinline__ int* fin_entry(const RkfArgs& a, int cls, long long i) {
+  return cls == 1 ? &a.elist[a.n - 1 - i] : (cls == 2 ? &a.elist2[a.n - 1 - i] : &a.elist2[i]);
+}
+
+// Longest first: the finisher lists 1 / 2 sorted by predicted remaining attempts, descending (one CTA; rank sort in
+// shared memory, n <= RKF_ORDER_MAX).  A straggler that starts late ends late; the order costs nothing else.
+constexpr int RKF_ORDER_MAX = 6144;
+__global__ void __launch_bounds__(1024) rkf_order_kernel(const RkfArgs a, const int cls) {
+  extern __shared__ double sm[];
+  const int n = (int)fin_count(a, cls);
+  if (n < 2 || n > RKF_ORDER_MAX) return;
+  double* key = sm;
+  int* id = reinterpret_cast<int*>(sm + RKF_ORDER_MAX);
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    const int r = *fin_entry(a, cls, i);
+    id[i] = r;
+    key[i] = (a.dt - a.rec_t[r]) / a.rec_h[r];
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += blockDim.x) {
+    const double k = key[i];
+    int rank = 0;
+    for (int j = 0; j < n; ++j) rank += (key[j] > k || (key[j] == k && j < i)) ? 1 : 0;
+    *fin_entry(a, cls, rank) = id[i];
+  }
+}
+
+}  // namespace ck
+#include "ck_rkf_wide.cuh"
+namespace ck {
+
+// Lists too long for the rank sort are ordered coarsely: four buckets by predicted remaining attempts, descending (order
+// inside a bucket is arbitrary).  which = -1: the list of the resumed thread-per-reactor phase (front of elist; a reactor
+// that needs 1000 more attempts and is fetched last would add a second to the run), buckets at top / 2, / 4, / 8 with
+// top = mid_steps; which = 2: the middle class, top = big_steps.  One CTA; `tmp` (n ints) is the buffer.
+__global__ void __launch_bounds__(1024) rkf_bucket_kernel(const RkfArgs a, const int which, int* __restrict__ tmp) {
+  __shared__ int cnt[4], cur[4];
+  const int n = (int)(which < 0 ? a.stats->n_evicted : fin_count(a, which));
+  const double top = which < 0 ? a.mid_steps : a.big_steps;
+  if (threadIdx.x < 4) cnt[threadIdx.x] = 0;
+  __syncthreads();
+  auto entry = [&](int i) -> int* { return which < 0 ? &a.elist[i] : fin_entry(a, which, i); };
+  auto bucket = [&](int r) {
+    const double pred = (a.dt - a.rec_t[r]) / a.rec_h[r];
+    return pred > 0.5 * top ? 0 : (pred > 0.25 * top ? 1 : (pred > 0.125 * top ? 2 : 3));
+  };
+  for (int i = threadIdx.x; i < n; i += blockDim.x) atomicAdd(&cnt[bucket(*entry(i))], 1);
+  __syncthreads();
+  if (threadIdx.x == 0) { cur[0] = 0; cur[1] = cnt[0]; cur[2] = cnt[0] + cnt[1]; cur[3] = cnt[0] + cnt[1] + cnt[2]; }
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += blockDim.x) { const int r = *entry(i); tmp[atomicAdd(&cur[bucket(r)], 1)] = r; }
+  __syncthreads();
+  for (int i = threadIdx.x; i < n; i += blockDim.x) *entry(i) = tmp[i];
+}
 
 enum { ST_H0A = -2, ST_H0B = -1 };  // EstimateH0 evaluations; 0..5 = RK stages
 
@@ -114,8 +179,12 @@ __global__ void __launch_bounds__(BLOCK, 1) rkf45_kernel(const MechDev m, const 
         // classification: reactors whose predicted number of remaining attempts (t_f - t) / h is large are the critical
         // chains of the batch -- they go to the wide, latency-optimised finisher AT ONCE (it runs beside the resumed
         // thread-per-reactor phase of everybody else)
-        if ((a.dt - t) > a.big_steps * h) a.elist[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_b, 1ULL)] = (int)r;
+        const double pred = fmin((a.dt - t) / h, 1e9);
+        const int kind = (pred > a.big_steps) ? 2 : ((pred > a.mid_steps) ? 1 : 0);
+        if (kind == 2) a.elist[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_b, 1ULL)] = (int)r;
+        else if (kind == 1) a.elist2[a.n - 1 - (long long)atomicAdd(&a.stats->n_evicted_m, 1ULL)] = (int)r;
         else a.elist[atomicAdd(&a.stats->n_evicted, 1ULL)] = (int)r;
+        atomicAdd(&a.stats->sum_pred[kind], (unsigned long long)pred);
       } else {
         a.elist2[atomicAdd(&a.stats->n_evicted_n, 1ULL)] = (int)r;   // end-game: the throughput-oriented finisher
       }
@@ -275,8 +344,7 @@ __host__ __device__ inline size_t rkf_coop_smem_doubles(int K, int R, int n_tent
   return (size_t)8 * (K + 1) + coop_chem_doubles(K, R, false) + (size_t)((n_tent + K + 2 + 1) >> 1);
 }
 
-// WIDE: the latency-optimised evaluation rhs_wide (G = 384 threads, one reaction per thread for R <= 384)
-template <int G, bool WIDE>
+template <int G>
 __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const RkfArgs a, const int cls) {
   extern __shared__ double sm[];
   __shared__ long long s_next;
@@ -285,24 +353,14 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
   double* F = sm + N;        // six evaluation vectors F[j*N + c]
   double* YT = sm + 7 * N;   // stage argument / candidate
   CoopChem c = coop_carve(sm + 8 * N, m.K, m.R, false);
-  if (WIDE) {  // the gather lists of rhs_wide, staged once per CTA
-    int* s_tptr = reinterpret_cast<int*>(sm + 8 * N + coop_chem_doubles(m.K, m.R, false));
-    int* s_tent = s_tptr + m.K + 1;
-    for (int i = tid; i <= m.K; i += G) s_tptr[i] = __ldg(m.tptr + i);
-    for (int i = tid; i < m.n_tent; i += G) s_tent[i] = __ldg(m.tent + i);
-    c.tptr = s_tptr; c.tent = s_tent;
-    __syncthreads();
-  }
-  WideRegs wr;
-  if constexpr (WIDE) wide_setup<G>(m, wr);
-  const long long n_ev = (long long)(cls ? a.stats->n_evicted_b : a.stats->n_evicted_n);
+  const long long n_ev = fin_count(a, cls);
   unsigned long long c_rhs = 0, c_att = 0, c_acc = 0, c_rej = 0, c_fail = 0;
   for (;;) {
     __syncthreads();
-    if (tid == 0) s_next = (long long)atomicAdd(cls ? &a.stats->queue_b : &a.stats->queue2, 1ULL);
+    if (tid == 0) s_next = (long long)atomicAdd(fin_queue(a, cls), 1ULL);
     __syncthreads();
     if (s_next >= n_ev) break;
-    const long long r = cls ? a.elist[a.n - 1 - s_next] : a.elist2[s_next];
+    const long long r = *fin_entry(a, cls, s_next);
     const double p = a.p[r];
     for (int i = tid; i < N; i += G) Y[i] = a.y[(size_t)i * a.ld + r];
     double t = a.rec_t[r], h = a.rec_h[r], fac_max = a.rec_fac[r], h_used = 0.0;
@@ -315,8 +373,7 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
       bool last = false;
       if (h >= a.dt - t) { h = a.dt - t; last = true; }
       TState ts;
-      if constexpr (WIDE) rhs_wide<G>(m, Y, p, F, c, ts, wr);
-      else rhs_coop<G, false>(m, Y, p, F, c, ts);
+      rhs_coop<G, false>(m, Y, p, F, c, ts);
       for (int s = 0; s < 5; ++s) {
         for (int i = tid; i < N; i += G) {
           double acc = 0.0;
@@ -324,8 +381,7 @@ __global__ void __launch_bounds__(G) rkf45_coop_kernel(const MechDev m, const Rk
           YT[i] = fma(h, acc, Y[i]);
         }
         __syncthreads();
-        if constexpr (WIDE) rhs_wide<G>(m, YT, p, F + (s + 1) * N, c, ts, wr);
-        else rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
+        rhs_coop<G, false>(m, YT, p, F + (s + 1) * N, c, ts);
       }
       c_rhs += 6;
       double es = 0.0;
@@ -439,22 +495,27 @@ int32_t launch_main(const ck_mech* m, const RkfPlan& pl, const RkfArgs& a, long 
 }
 }  // namespace
 
-// workspace: [DevStats][int attempts[n]][hand-over: 4 int + 3 double per reactor][double V[8][N][slots]]
+// workspace: [DevStats][int attempts[n]][hand-over: 5 int + 3 double per reactor][double V[8][N][slots]]
 size_t ck_rkf_workspace(const ck_mech* m, int64_t n) {
   if (n == 0) return sizeof(DevStats);
   RkfPlan pl;
   if (rkf_plan(m, n, &pl) != CK_OK) return sizeof(DevStats);  // the integrate call reports the error
-  return sizeof(DevStats) + 5 * al256((size_t)n * sizeof(int)) + 3 * al256((size_t)n * sizeof(double)) +
+  return sizeof(DevStats) + 6 * al256((size_t)n * sizeof(int)) + 3 * al256((size_t)n * sizeof(double)) +
          (size_t)8 * (m->K + 1) * rkf_vslots(pl, n) * sizeof(double);
 }
 
 // Flow (flags = 0, models with N > 32):
 //   1  classification: the thread-per-reactor kernel over all reactors, every reactor handed on after RKF_CAP attempts
-//      (most of config 4's reactors need more); predicted stragglers -> list W, the others -> list C
-//   2a the wide finisher over list W on a SECOND stream, one 384-thread CTA per straggler (their serial chains are the
-//      critical path, so they start now and run beside 2b / 3)
-//   2b the thread-per-reactor kernel resumes list C (lane refill; end-game eviction -> list N)
-//   3  the narrow finisher over list N (64 / 128-thread CTAs, many per SM)
+//      (most of config 4's reactors need more) into one of three lists by its predicted remaining attempts (t_f - t) / h:
+//      stragglers (> RKF_BIG), middle class (> RKF_MID), the rest
+//   2a the wide finisher over the stragglers, longest first, one 384-thread CTA and one SM per straggler: their serial
+//      chains are the critical path of the batch (ck_rkf_wide.cuh: 18 us per attempt against 0.8-1 ms thread-per-reactor)
+//   2b the thread-per-reactor kernel resumes the rest, long ones first (lane refill; end-game eviction -> list N): the
+//      cheapest mode per attempt (2.1 us of an SM), usable only where ~1 ms per attempt does not make the reactor late
+//   2c the narrow finisher over the middle class, longest first (64 / 128-thread CTAs, eight per SM: 7.4 us of an SM per
+//      attempt, 40-60 us per attempt for one reactor)
+//      2a, 2b and 2c run side by side on three streams over disjoint SMs (shares from the predicted work, see below)
+//   3  the narrow finisher over list N
 // N <= 32: phases 1 (uncapped, with end-game eviction) and 3 only.  flags bit 0 / 1: one kernel, no eviction.
 extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, int64_t ld, const double* p, double dt,
                                       const ck_opts* o, int32_t* n_accept, int32_t* n_reject, int32_t* status,
@@ -465,7 +526,7 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   if (n > 0) { int32_t rc0 = rkf_plan(m, n, &pl); if (rc0) return rc0; }
   const size_t nslots = n > 0 ? rkf_vslots(pl, n) : 0;
   const size_t bi = al256((size_t)n * sizeof(int)), bd = al256((size_t)n * sizeof(double));
-  const size_t need = n > 0 ? sizeof(DevStats) + 5 * bi + 3 * bd + (size_t)8 * (m->K + 1) * nslots * sizeof(double) : sizeof(DevStats);
+  const size_t need = n > 0 ? sizeof(DevStats) + 6 * bi + 3 * bd + (size_t)8 * (m->K + 1) * nslots * sizeof(double) : sizeof(DevStats);
   int32_t rc = integrate_prologue("ck_integrate_rkf45", m, n, y, ld, p, dt, o, ws, ws_bytes, need, st);
   if (rc) return rc;
   if (n == 0) { if (report) *report = ck_report{}; return CK_OK; }
@@ -479,6 +540,7 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   a.att = (int*)wp; wp += bi;
   a.elist = (int*)wp; wp += bi;
   a.elist2 = (int*)wp; wp += bi;
+  a.tmp = (int*)wp; wp += bi;
   a.rec_acc = (int*)wp; wp += bi;
   a.rec_rej = (int*)wp; wp += bi;
   a.rec_t = (double*)wp; wp += bd;
@@ -488,70 +550,129 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
   const bool finishers = !(o->flags & 3);          // bit 0: static mapping, bit 1: refill only (no finisher)
   const bool classify = finishers && N > 32;
   constexpr int RKF_CAP = 24;                       // attempts before a reactor is classified
-  constexpr double RKF_BIG = 12000.0;               // predicted remaining attempts that make a straggler
+  constexpr double RKF_BIG = 8000.0;                // predicted remaining attempts that make a straggler (wide finisher)
+  constexpr double RKF_MID = 400.0;                 // ... that send a reactor to the narrow finisher at once
   a.rlist = nullptr; a.rcount = nullptr; a.rqueue = &a.stats->queue;
   a.cap = classify ? std::min(RKF_CAP, a.max_steps) : 0;
-  a.big_steps = RKF_BIG;
+  a.big_steps = (o->flags & 16) ? -1.0 : RKF_BIG;   // bit 4 (measurement): every classified reactor counts as a straggler
+  // small batches cannot fill the lanes of the thread-per-reactor kernel, whose ~1 ms per attempt then is all they would
+  // get from it: everything goes to the finishers after the classification pass (n = 4096: 0.4 s instead of 1.9 s)
+  a.mid_steps = (n < 16384) ? -1.0 : RKF_MID;
   a.evict = (finishers && !classify) ? 1 : 0;
   // everything the finishers need is validated BEFORE the first launch: a failure must not leave y half-integrated
   const size_t smem2 = rkf_coop_smem_doubles(m->K, m->R, m->dev.n_tent) * sizeof(double);
   if (finishers && smem2 > 227 * 1024) { set_error("ck_integrate_rkf45: mechanism too large for the cooperative finisher"); return CK_EUNSUPPORTED; }
   int sms = 0;
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
+  if (finishers) {
+    // Touch every kernel of the flow BEFORE the first launch: CUDA loads kernels lazily, and a first-use load issued while
+    // another kernel runs waits for it -- the side-by-side phases of the first call of a process would run one after
+    // the other (measured: 3.4 s instead of 1.45 s for config 4).
+    cudaFuncAttributes fa;
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_wide_kernel<WIDE_G>));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<32>));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<64>));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<128>));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf_order_kernel));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf_bucket_kernel));
+    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_kernel<512, true>));
+  }
   rc = launch_main(m, pl, a, pl.grid, st);
   if (rc) return rc;
   int rounds = 1;
   if (finishers) {
     int per_sm = 0;
-    auto launch_fin = [&](auto kern, int G, int cls, long long want, cudaStream_t s) -> int32_t {
-      CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
-      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G, smem2));
+    auto launch_fin = [&](auto kern, int G, int cls, long long want, cudaStream_t s, size_t smem = 0) -> int32_t {
+      if (smem == 0) smem = smem2;
+      CK_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+      CK_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, G, smem));
       const long long grid = std::max<long long>(1, std::min<long long>(want, (long long)std::max(per_sm, 1) * sms));
-      kern<<<(unsigned)grid, G, smem2, s>>>(m->dev, a, cls);
+      kern<<<(unsigned)grid, G, smem, s>>>(m->dev, a, cls);
       CK_CUDA(cudaGetLastError());
       return CK_OK;
     };
-    cudaStream_t s2 = nullptr;
-    cudaEvent_t ev_fin = nullptr;
+    cudaStream_t s2 = nullptr, s3 = nullptr;
+    cudaEvent_t ev_fin = nullptr, ev_fin3 = nullptr;
     if (classify) {
-      DevStats hs;   // the two list lengths size the next launches (one small read-back; this call synchronises anyway)
+      DevStats hs;   // the list lengths size the next launches (one small read-back; this call synchronises anyway)
       CK_CUDA(cudaMemcpyAsync(&hs, a.stats, sizeof hs, cudaMemcpyDeviceToHost, st));
       CK_CUDA(cudaStreamSynchronize(st));
-      const long long nW = (long long)hs.n_evicted_b, nC = (long long)hs.n_evicted;
-      if (nW > 0) {   // 2a: the stragglers, beside everything that follows
-        cudaEvent_t ev_main = nullptr;
-        CK_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+      const long long nW = (long long)hs.n_evicted_b, nM = (long long)hs.n_evicted_m, nC = (long long)hs.n_evicted;
+      const size_t smem_w = rkf_wide_smem_doubles(m->K, m->R, m->dev.r_tb, m->dev.n_tent) * sizeof(double);
+      const bool wide_ok = m->K <= 128 && smem_w <= 227 * 1024 && !(o->flags & 32);
+      // SM shares.  The three phases that follow run side by side, and the resumed thread-per-reactor kernel and the wide
+      // finisher each need a whole SM per CTA, so the split is made here: the stragglers get one SM each (at most 40 % of
+      // the machine), the rest is divided between the resumed kernel and the narrow finisher in proportion to their
+      // predicted work (measured cost per attempt: 2.1 us of an SM thread-per-reactor, 7.4 us on narrow CTAs); the narrow
+      // finisher is launched with more CTAs than fit, so it also takes over every SM the other two give back.
+      const long long gW = std::min<long long>(nW, (nC + nM > 0) ? (2 * sms) / 5 : sms);
+      const double eb = 2.1 * (double)hs.sum_pred[0], em = 7.4 * (double)hs.sum_pred[1];
+      const long long rem = sms - (wide_ok ? gW : 0);
+      long long gC = rem;
+      if (nM > 0 || (nW > 0 && !wide_ok)) gC = std::max<long long>(8, std::min<long long>(rem - 8, (long long)((double)rem * eb / std::max(eb + em, 1.0) + 0.5)));
+      cudaEvent_t ev_main = nullptr;
+      if (nW > 0 || nM > 0) {
         CK_CUDA(cudaEventCreateWithFlags(&ev_main, cudaEventDisableTiming));
-        CK_CUDA(cudaEventCreateWithFlags(&ev_fin, cudaEventDisableTiming));
         CK_CUDA(cudaEventRecord(ev_main, st));
+      }
+      if (nC > 0) {   // 2b: resume the rest thread-per-reactor (first: its CTAs take their SMs before the others are placed)
+        RkfPlan pl2;
+        rc = rkf_plan(m, nC, &pl2);
+        if (rc) return rc;
+        rkf_bucket_kernel<<<1, 1024, 0, st>>>(a, -1, a.tmp);
+        RkfArgs ac = a;
+        ac.cap = 0; ac.evict = 1;
+        ac.rlist = a.elist; ac.rcount = &a.stats->n_evicted; ac.rqueue = &a.stats->queue_c;
+        rc = launch_main(m, pl2, ac, std::min<long long>(pl2.grid, gC), st);
+        if (rc) return rc;
+        rounds++;
+      }
+      const int order_smem = RKF_ORDER_MAX * 12;
+      if (nW > 0) {   // 2a: the stragglers, longest first
+        CK_CUDA(cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking));
+        CK_CUDA(cudaEventCreateWithFlags(&ev_fin, cudaEventDisableTiming));
         CK_CUDA(cudaStreamWaitEvent(s2, ev_main, 0));
-        rc = launch_fin(rkf45_coop_kernel<384, true>, 384, 1, nW, s2);
-        cudaEventDestroy(ev_main);
+        CK_CUDA(cudaFuncSetAttribute(rkf_order_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, order_smem));
+        rkf_order_kernel<<<1, 1024, order_smem, s2>>>(a, 1);
+        if (wide_ok) rc = launch_fin(rkf45_wide_kernel<WIDE_G>, WIDE_G, 1, gW, s2, smem_w);
+        else rc = (N <= 64) ? launch_fin(rkf45_coop_kernel<64>, 64, 1, nW, s2) : launch_fin(rkf45_coop_kernel<128>, 128, 1, nW, s2);
         if (rc) return rc;
         CK_CUDA(cudaEventRecord(ev_fin, s2));
         rounds++;
       }
-      if (nC > 0) {   // 2b: resume the rest thread-per-reactor
-        RkfPlan pl2;
-        rc = rkf_plan(m, nC, &pl2);
+      if (nM > 0) {   // 2c: the middle class on narrow CTAs, longest first, oversubscribed
+        CK_CUDA(cudaStreamCreateWithFlags(&s3, cudaStreamNonBlocking));
+        CK_CUDA(cudaEventCreateWithFlags(&ev_fin3, cudaEventDisableTiming));
+        CK_CUDA(cudaStreamWaitEvent(s3, ev_main, 0));
+        CK_CUDA(cudaFuncSetAttribute(rkf_order_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, order_smem));
+        if (nM <= RKF_ORDER_MAX) rkf_order_kernel<<<1, 1024, order_smem, s3>>>(a, 2);
+        else rkf_bucket_kernel<<<1, 1024, 0, s3>>>(a, 2, a.tmp + nC);   // the two bucket passes may overlap: disjoint halves
+        if (wide_ok && nC == 0 && nW + nM <= sms)   // SMs to spare: everybody gets the low-latency kernel
+          rc = launch_fin(rkf45_wide_kernel<WIDE_G>, WIDE_G, 2, nM, s3, smem_w);
+        else
+          rc = (N <= 64) ? launch_fin(rkf45_coop_kernel<64>, 64, 2, nM, s3) : launch_fin(rkf45_coop_kernel<128>, 128, 2, nM, s3);
         if (rc) return rc;
-        a.cap = 0; a.evict = 1;
-        a.rlist = a.elist; a.rcount = &a.stats->n_evicted; a.rqueue = &a.stats->queue_c;
-        rc = launch_main(m, pl2, a, pl2.grid, st);
-        if (rc) return rc;
+        CK_CUDA(cudaEventRecord(ev_fin3, s3));
         rounds++;
       }
+      if (ev_main) cudaEventDestroy(ev_main);
+      a.cap = 0; a.evict = 1;
     }
     // 3: whatever the end-game evicted (its count is read on the device)
-    if (N <= 32) rc = launch_fin(rkf45_coop_kernel<32, false>, 32, 0, n, st);
-    else if (N <= 64) rc = launch_fin(rkf45_coop_kernel<64, false>, 64, 0, n, st);
-    else rc = launch_fin(rkf45_coop_kernel<128, false>, 128, 0, n, st);
+    if (N <= 32) rc = launch_fin(rkf45_coop_kernel<32>, 32, 0, n, st);
+    else if (N <= 64) rc = launch_fin(rkf45_coop_kernel<64>, 64, 0, n, st);
+    else rc = launch_fin(rkf45_coop_kernel<128>, 128, 0, n, st);
     if (rc) return rc;
     rounds++;
-    if (s2) {   // join the second stream; both objects are released once their work has drained
+    if (s2) {   // join the side streams; the objects are released once their work has drained
       CK_CUDA(cudaStreamWaitEvent(st, ev_fin, 0));
       cudaEventDestroy(ev_fin);
       cudaStreamDestroy(s2);
+    }
+    if (s3) {
+      CK_CUDA(cudaStreamWaitEvent(st, ev_fin3, 0));
+      cudaEventDestroy(ev_fin3);
+      cudaStreamDestroy(s3);
     }
   }
   return integrate_report(m, n, a.att, a.stats, rounds, 0, report, st);

@@ -15,8 +15,11 @@ struct DevStats {
   unsigned long long n_evicted;    // reactors the capped classification phase hands on to the resumed thread-per-reactor phase
   unsigned long long queue2;       // work-queue head of the finisher
   unsigned long long qempty;       // set once the main queue ran dry
-  unsigned long long clk[8];       // ROS4 phase clocks (SM cycles summed over CTAs): 0 RHS+dq, 1 Jacobian assembly,
-                                   // 2 LU, 3 solves, 4 stage RHS, 5 vectors/control, 6 total
+  unsigned long long n_evicted_m;  // RKF45 classification: reactors of the middle class (narrow finisher, started at once;
+                                   // listed from the back of the second eviction list)
+  unsigned long long queue_m;      // work-queue head of that finisher
+  unsigned long long sum_pred[3];  // predicted remaining attempts summed per class: 0 resumed, 1 middle, 2 stragglers
+  unsigned long long spare[3];
   unsigned long long n_evicted_b;  // ... of which predicted stragglers (handed to the wide low-latency finisher; listed from
                                    // the back of the eviction list)
   unsigned long long queue_b;      // work-queue head of the wide finisher
