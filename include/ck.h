@@ -78,7 +78,10 @@ typedef struct {
                           (measurement of the finishers): every reactor counts as a straggler after the classification
                           pass / the stragglers run on the narrow finisher instead of the wide one.
                           ROS4, bit 2: force the fused CTA-per-reactor kernel, bit 3: force the batched rounds
-                          (default: rounds for n >= 16384 reactors of a model with 33 <= N <= 128, analytic Jacobian). */
+                          (default: rounds for n >= 16384 reactors of a model with 33 <= N <= 128, analytic Jacobian),
+                          bit 6 (measurement): the rounds evaluate a fresh Jacobian for EVERY attempt; by default they keep
+                          f(y_n) and J(y_n) across a rejected attempt (y_n has not moved: same values, fewer evaluations,
+                          so jac_evals <= attempts and rhs_evals = 2 attempts + jac_evals + 2 n). */
 } ck_opts;
 
 /* Batch totals and divergence statistics, filled on the HOST after the call (may be NULL).

@@ -91,7 +91,7 @@ extern "C" int32_t ck_jac_batched_static(const ck_mech* m, int64_t n, const doub
   CK_CUDA(cudaSetDevice(m->device));
   cudaStream_t st = (cudaStream_t)stream;
   const size_t N = m->K + 1;
-  JacOut o;
+  JacOut o{};
   o.f = base; o.ldf = n;
   o.hc = o.f + al32(N * (size_t)n); o.ldh = n;
   o.g2 = o.hc + al32((size_t)jac_hc_rows(m->K) * n); o.ldg = n;

@@ -90,8 +90,9 @@ struct JacOut {
   long long sstride;  // ... and doubles per slot
   double* hc;       // [2K + 1][ldh]  hh_k, cc_k, and the constant of d f_T / d T
   long long ldh;
-  double* g2;       // [jac_g2_rows][ldg] scratch
+  double* g2;       // [jac_g2_rows][ldg] scratch (indexed by thread)
   long long ldg;
+  const int* list;  // null: thread i works on column i; else on column list[i] of y / p / f / hc / J
 };
 
 // phase A for one row of kind TYPE: rate of progress with derivative pieces, omega scatter, G2 stores
@@ -127,13 +128,13 @@ __device__ __forceinline__ void jac_phaseA_row(const MechDev& m, int r, const do
 // yin / out pointers are pre-offset to this thread's slot (component-major arrays) resp. reactor (Jrm).
 template <int BLOCK, bool RM>
 __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
-                                                const JacOut& o, long long slot, double* __restrict__ Cs, uint32_t wt,
+                                                const JacOut& o, long long slot, long long gslot, double* __restrict__ Cs, uint32_t wt,
                                                 double* __restrict__ stage, bool store) {
   const int K = m.K, R = m.R, rs = m.rstride, N = K + 1;
   const int tid = threadIdx.x;
   const TState t = make_tstate(m, yin[0]);
   double* const fout = o.f + slot;
-  double* const g2 = o.g2 + slot;
+  double* const g2 = o.g2 + gslot;   // the scratch is indexed by thread, the outputs by column
   double* const hc = o.hc + slot;
   // ---- phase A: f(y) (as rhs_thread_tmem) ----------------------------------------------------------------------
   double S = 0.0, cps = 0.0, dcp = 0.0;
@@ -397,10 +398,11 @@ __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, lon
     const long long r = b * BLOCK + tid;
     const bool act = r < n;
     const long long rr = act ? r : n - 1;
+    const long long col = o.list ? (long long)o.list[rr] : rr;   // which column of y / p / f / hc / J this thread works on
     JacOut oo = o;
-    if (RM) oo.J = o.J + (size_t)rr * o.sstride;
-    else oo.J = o.J + rr;
-    jac_thread_tmem<BLOCK, RM>(m, y + rr, ld, p[rr], oo, rr, Cs, wt, stage, act);
+    if (RM) oo.J = o.J + (size_t)col * o.sstride;
+    else oo.J = o.J + col;
+    jac_thread_tmem<BLOCK, RM>(m, y + col, ld, p[col], oo, col, rr, Cs, wt, stage, act);
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();

@@ -412,7 +412,7 @@ int32_t integrate_report(const ck_mech* m, int64_t n, const int32_t* att_dev, co
   CK_CUDA(cudaStreamSynchronize(st));
   rep->attempts = (int64_t)hs.attempts; rep->accepted = (int64_t)hs.accepted; rep->rejected = (int64_t)hs.rejected;
   rep->rhs_evals = (int64_t)hs.rhs_evals; rep->jac_evals = (int64_t)hs.jac_evals;
-  rep->lu_factor = (int64_t)hs.jac_evals * lu_per_jac;
+  rep->lu_factor = (int64_t)hs.attempts * lu_per_jac;   // one factorisation per attempt (the Jacobian may be older: ck_ros_rounds.cu)
   rep->simt_efficiency = hs.lane_total ? (double)hs.lane_active / (double)hs.lane_total : 1.0;
   rep->waste_p32 = waste_static(att, 32);
   rep->rounds = rounds;

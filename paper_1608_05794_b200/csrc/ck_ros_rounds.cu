@@ -11,8 +11,10 @@
 // streamed in from HBM once per attempt.  One attempt round:
 //
 //   gather     Yw[:, s] = y[:, act[s]]                                              (thread per slot)
-//   jac_rows   f0 = f(Yw), species rows of J, pieces of row 0        -> F0, LU buffer, HC     (thread per slot)
-//   lu         row 0, A = I/(h gamma) - J, P A = L U, u1 = A^-1 f0, YT = y + a21 u1           (2-4 warps per slot)
+//   jac_rows   f0 = f(y), species rows of J, pieces of row 0 -> F0, JB, HC, all indexed by REACTOR; only for the
+//              reactors whose state changed since their last Jacobian -- after a REJECTED attempt y_n, hence f(y_n)
+//              and J(y_n), are what they were (a third of config 3's attempts), only h changes          (thread per reactor)
+//   lu         row 0, A = I/(h gamma) - J, P A = L U (-> LU, per slot), u1 = A^-1 f0, YT = y + a21 u1   (2-4 warps per slot)
 //   ck_rhs     FT = f(YT)                                                                     (thread per slot)
 //   solve2     u2 = A^-1 (FT + c21/h u1), YT = y + a31 u1 + a32 u2                            (2-4 warps per slot)
 //   ck_rhs     FT = f(YT)
@@ -47,12 +49,19 @@ struct RoundArgs {
   int *nacc, *nrej;
   // active lists and counters: cnt[0] = active now, cnt[1] = appended for the next round
   int *act, *act2, *cnt;
+  // need[r]: bit 0 = active in the next round, bit 1 = needs a fresh Jacobian; compacted IN REACTOR ORDER into act2 / jl2
+  // (cnt[1] / cnt[3]) -- an atomic append would scatter neighbouring threads over the whole matrix array (measured: +60 %
+  // on the Jacobian kernel)
+  int *jl, *jl2, *need;
+  int always_jac;   // measurement (flags bit 6): a fresh Jacobian for every attempt, as the fused kernel does
   // per-slot arrays
-  double *Yw, *Pw, *F0, *YT, *FT;  // component-major [N][cap] ([cap] for Pw)
+  double *Yw, *Pw, *YT, *FT;       // component-major [N][cap] ([cap] for Pw)
+  double* F0;                      // [N][cap] f(y_n), indexed by REACTOR (kept across a rejected attempt)
   double *U1, *U2;                 // reactor-major [cap][N]
-  double* HC;                      // [2K+1][cap]
+  double* HC;                      // [2K+1][cap], indexed by REACTOR
   double* G2;                      // [g2rows][cap]
-  double* LU;                      // [cap][lu_stride]: species rows of J, then L\U (row stride lu_ldr)
+  double* JB;                      // [cap][lu_stride]: species rows of -J in the layout of the factorisation, by REACTOR
+  double* LU;                      // [cap][lu_stride]: L\U of this attempt, by slot (row stride lu_ldr)
   long long lu_stride;
   int lu_ldr;
   double* dinv;                    // [cap][N]
@@ -64,11 +73,12 @@ struct RoundArgs {
 
 __global__ void ros_init_kernel(RoundArgs a) {
   const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (r == 0) { a.cnt[0] = (int)a.n; a.cnt[1] = 0; }
+  if (r == 0) { a.cnt[0] = (int)a.n; a.cnt[1] = 0; a.cnt[2] = 0; a.cnt[3] = 0; }
   if (r >= a.n) return;
   a.act[r] = (int)r;
   a.t[r] = 0.0; a.h[r] = a.h0; a.fac[r] = 5.0;
   a.nacc[r] = 0; a.nrej[r] = 0;
+  a.need[r] = 0;
 }
 
 __global__ void ros_gather_kernel(RoundArgs a, int N) {
@@ -122,7 +132,7 @@ __global__ void ros_guard_kernel(RoundArgs a) {
   if (a.max_steps <= 0) st = CK_ST_MAX_STEPS;
   else if (!isfinite(h)) st = CK_ST_NONFINITE;
   else if (h < 1e-12 * a.dt) st = CK_ST_H_UNDERFLOW;
-  if (st == CK_ST_OK) { a.act2[atomicAdd(&a.cnt[1], 1)] = r; return; }
+  if (st == CK_ST_OK) { a.need[r] = 3; return; }
   if (a.n_accept) a.n_accept[r] = 0;
   if (a.n_reject) a.n_reject[r] = 0;
   if (a.status) a.status[r] = st;
@@ -130,7 +140,31 @@ __global__ void ros_guard_kernel(RoundArgs a) {
   a.att[r] = 0;
   atomicAdd(&a.stats->failed, 1ULL);
 }
-__global__ void ros_swap_kernel(RoundArgs a) { a.cnt[0] = a.cnt[1]; a.cnt[1] = 0; }
+// need[] -> act2 (bit 0: active in the next round) and jl2 (bit 1: needs a fresh Jacobian), both ascending inside a block of
+// 1024 reactors (blocks land in the order of their atomics): slots and matrix blocks stay in reactor order
+__global__ void __launch_bounds__(1024) ros_lists_kernel(RoundArgs a) {
+  __shared__ int wsum[2][32];
+  __shared__ int base[2];
+  const long long r = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int flg = r < a.n ? a.need[r] : 0;
+  const unsigned b0 = __ballot_sync(0xffffffffu, flg & 1), b1 = __ballot_sync(0xffffffffu, flg & 2);
+  if (lane == 0) { wsum[0][warp] = __popc(b0); wsum[1][warp] = __popc(b1); }
+  __syncthreads();
+  if (warp < 2) {
+    const int v = wsum[warp][lane];
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    wsum[warp][lane] = x - v;
+    if (lane == 31) base[warp] = x > 0 ? atomicAdd(&a.cnt[warp == 0 ? 1 : 3], x) : 0;
+  }
+  __syncthreads();
+  const unsigned below = (1u << lane) - 1u;
+  if (flg & 1) a.act2[base[0] + wsum[0][warp] + __popc(b0 & below)] = (int)r;
+  if (flg & 2) a.jl2[base[1] + wsum[1][warp] + __popc(b1 & below)] = (int)r;
+}
+__global__ void ros_swap_kernel(RoundArgs a) { a.cnt[0] = a.cnt[1]; a.cnt[1] = 0; a.cnt[2] = a.cnt[3]; a.cnt[3] = 0; }
 
 // ---- warp-per-reactor kernels: blocked DMMA LU and shuffle solves (ck_lu_warp.cuh); CTA = one warp = one slot ------
 // The slot's block in HBM is the shared-memory image of the matrix (luw_np(N) rows of stride luw_lda(N)): it moves
@@ -160,16 +194,16 @@ __device__ __forceinline__ void rw_copy_block(double* __restrict__ dst, const do
 }
 // the slot's matrix block -> shared memory as ONE bulk copy (the caller has made sure that nobody still uses sh.A and waits
 // on `bar` with the current parity before reading it)
-__device__ __forceinline__ void rw_issue_block_load(const RoundArgs& a, long long s, int N, const RwShared& sh, uint64_t* bar) {
+__device__ __forceinline__ void rw_issue_block_load(const double* __restrict__ src, int N, const RwShared& sh, uint64_t* bar) {
   if (threadIdx.x == 0) {
     fence_async_smem();
-    bulk_load(sh.A, a.LU + (size_t)s * a.lu_stride, (uint32_t)(luw_block_doubles(N) * sizeof(double)), bar);
+    bulk_load(sh.A, src, (uint32_t)(luw_block_doubles(N) * sizeof(double)), bar);
   }
 }
 template <int RWT>
 __device__ __forceinline__ void rw_load_factors(const RoundArgs& a, long long s, int N, const RwShared& sh, uint64_t* bar, uint32_t parity) {
   const int tid = threadIdx.x;
-  rw_issue_block_load(a, s, N, sh, bar);
+  rw_issue_block_load(a.LU + (size_t)s * a.lu_stride, N, sh, bar);
   for (int i = tid; i < N; i += RWT) { sh.dinv[i] = a.dinv[(size_t)s * N + i]; sh.perm[i] = a.pst[(size_t)s * N + i]; }
   mbar_wait(bar, parity);
 }
@@ -191,10 +225,10 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
     if (tid == 0) bulk_store_wait_read();   // the previous slot's factors have left shared memory
     __syncthreads();
     double* blk = a.LU + (size_t)s * a.lu_stride;
-    // the slot's block (rows 1..K of -J, written by jac_rows_kernel in the image's layout) arrives as one bulk copy
-    rw_issue_block_load(a, s, N, sh, &s_bar);
-    for (int k = tid; k < K; k += RWT) { sh.v0[k] = a.HC[(size_t)k * a.cap + s]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + s]; }
-    for (int i = tid; i < N; i += RWT) sh.v2[i] = a.F0[(size_t)i * a.cap + s];
+    // the reactor's block (rows 1..K of -J, written by jac_rows_kernel in the image's layout) arrives as one bulk copy
+    rw_issue_block_load(a.JB + (size_t)r * a.lu_stride, N, sh, &s_bar);
+    for (int k = tid; k < K; k += RWT) { sh.v0[k] = a.HC[(size_t)k * a.cap + r]; sh.v1[k] = a.HC[(size_t)(K + k) * a.cap + r]; }
+    for (int i = tid; i < N; i += RWT) sh.v2[i] = a.F0[(size_t)i * a.cap + r];
     double h = a.h[r];
     const double trem = a.dt - a.t[r];
     int flg = 0;
@@ -209,7 +243,7 @@ __global__ void __launch_bounds__(32 * RW) ros_lu_w_kernel(RoundArgs a, int K) {
     __syncthreads();
     // row 0 of A = I/(h gamma) - J from the (negated) species rows (ck_jac_tpr.cuh): -J_0j = -sum_k hh_k M_kj + f_T cc_j
     const double fT = sh.v2[0];
-    const double jtt = a.HC[(size_t)(2 * K) * a.cap + s];
+    const double jtt = a.HC[(size_t)(2 * K) * a.cap + r];
     for (int j = tid; j < NP; j += RWT) {
       double acc0 = 0.0, acc1 = 0.0;
       int k = 0;
@@ -352,13 +386,14 @@ __global__ void __launch_bounds__(32 * RW) ros_solve34_w_kernel(RoundArgs a, int
     const double err = sqrt(es / N);
     double tcur = a.t[r], hn = h, fac_max = a.fac[r];
     int nacc = a.nacc[r], nrej = a.nrej[r], status = CK_ST_OK;
-    bool done = false;
+    bool done = false, accepted = false;
     if (flg & 2) { status = CK_ST_ZERO_PIVOT; done = true; }
     else if (isfinite(err) && err < 1.0) {
 #pragma unroll
       for (int q = 0; q < NR; ++q) { const int i = lane + 32 * q; if (i < N) a.y[(size_t)i * a.ld + r] = yn[q]; }
       tcur = (flg & 1) ? a.dt : tcur + h;
       nacc++;
+      accepted = true;
       hn = h * fmin(fac_max, fmax(0.2, 0.9 * pow(fmax(err, 1e-10), -0.25)));
       fac_max = 5.0;
       c_acc++;
@@ -382,9 +417,10 @@ __global__ void __launch_bounds__(32 * RW) ros_solve34_w_kernel(RoundArgs a, int
         if (a.status) a.status[r] = status;
         if (a.h_last) a.h_last[r] = (flg & 2) ? 0.0 : h;
         a.att[r] = nacc + nrej;
+        a.need[r] = 0;
         c_fail += (status != CK_ST_OK);
       } else {
-        a.act2[atomicAdd(&a.cnt[1], 1)] = r;
+        a.need[r] = (accepted || a.always_jac) ? 3 : 1;   // still active; y_n moved: f(y_n) and J(y_n) are due again
       }
     }
   }
@@ -412,7 +448,7 @@ inline long long rr_lu_stride(const ck_mech* m) {
 }
 
 struct RrLayout {
-  size_t att, t, h, fac, nacc, nrej, act, act2, cnt, Yw, Pw, F0, YT, FT, U1, U2, HC, G2, LU, dinv, pst, hs, flg, total;
+  size_t att, t, h, fac, nacc, nrej, act, act2, jl, jl2, need, cnt, Yw, Pw, F0, YT, FT, U1, U2, HC, G2, JB, LU, dinv, pst, hs, flg, total;
 };
 RrLayout rr_layout(const ck_mech* m, int64_t n) {
   const size_t N = m->K + 1, cap = (size_t)n;
@@ -422,11 +458,12 @@ RrLayout rr_layout(const ck_mech* m, int64_t n) {
   L.att = put(cap * 4);   // must follow the header: integrate_report reads it there
   L.t = put(cap * 8); L.h = put(cap * 8); L.fac = put(cap * 8);
   L.nacc = put(cap * 4); L.nrej = put(cap * 4);
-  L.act = put(cap * 4); L.act2 = put(cap * 4); L.cnt = put(64);
+  L.act = put(cap * 4); L.act2 = put(cap * 4); L.jl = put(cap * 4); L.jl2 = put(cap * 4); L.need = put(cap * 4); L.cnt = put(64);
   L.Yw = put(N * cap * 8); L.Pw = put(cap * 8); L.F0 = put(N * cap * 8); L.YT = put(N * cap * 8); L.FT = put(N * cap * 8);
   L.U1 = put(N * cap * 8); L.U2 = put(N * cap * 8);
   L.HC = put((size_t)jac_hc_rows(m->K) * cap * 8);
   L.G2 = put((size_t)jac_g2_rows(m->R, m->dev.r_tb) * cap * 8);
+  L.JB = put(cap * (size_t)rr_lu_stride(m) * 8);
   L.LU = put(cap * (size_t)rr_lu_stride(m) * 8);
   L.dinv = put(cap * N * 8); L.pst = put(cap * N * 4);
   L.hs = put(cap * 8); L.flg = put(cap * 4);
@@ -438,11 +475,12 @@ template <int BLOCK>
 int32_t launch_jac_rows_rm(const ck_mech* m, const RoundArgs& a, long long na, int sms, cudaStream_t st) {
   const size_t smem = jac_tpr_smem_bytes(m->K, m->R, m->dev.n_tent, m->dev.rstride, BLOCK);
   CK_CUDA(cudaFuncSetAttribute(jac_rows_kernel<BLOCK, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  JacOut o;
-  o.f = a.F0; o.ldf = a.cap; o.J = a.LU; o.ldJ = 0; o.ldr = a.lu_ldr; o.sstride = a.lu_stride;
+  JacOut o{};
+  o.f = a.F0; o.ldf = a.cap; o.J = a.JB; o.ldJ = 0; o.ldr = a.lu_ldr; o.sstride = a.lu_stride;
   o.hc = a.HC; o.ldh = a.cap; o.g2 = a.G2; o.ldg = a.cap;
+  o.list = a.jl;   // thread i works on reactor jl[i]: state straight from y, outputs by reactor
   const long long grid = std::max<long long>(1, std::min<long long>((na + BLOCK - 1) / BLOCK, sms));
-  jac_rows_kernel<BLOCK, true><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, na, a.cnt, a.Yw, a.cap, a.Pw, o);
+  jac_rows_kernel<BLOCK, true><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, na, a.cnt + 2, a.y, a.ld, a.p, o);
   CK_CUDA(cudaGetLastError());
   return CK_OK;
 }
@@ -494,25 +532,29 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   RoundArgs a{};
   a.n = n; a.ld = ld; a.cap = n; a.y = y; a.p = p; a.dt = dt; a.rtol = o->rtol; a.atol = o->atol; a.h0 = o->h0;
   a.max_steps = o->max_steps > 0 ? o->max_steps : 100000;
+  a.always_jac = (o->flags & 64) ? 1 : 0;
   a.n_accept = n_accept; a.n_reject = n_reject; a.status = status; a.h_last = h_last;
   a.stats = (DevStats*)ws;
   a.att = (int*)(w + L.att); a.t = (double*)(w + L.t); a.h = (double*)(w + L.h); a.fac = (double*)(w + L.fac);
   a.nacc = (int*)(w + L.nacc); a.nrej = (int*)(w + L.nrej); a.act = (int*)(w + L.act); a.act2 = (int*)(w + L.act2);
+  a.jl = (int*)(w + L.jl); a.jl2 = (int*)(w + L.jl2); a.need = (int*)(w + L.need);
   a.cnt = (int*)(w + L.cnt);
   a.Yw = (double*)(w + L.Yw); a.Pw = (double*)(w + L.Pw); a.F0 = (double*)(w + L.F0); a.YT = (double*)(w + L.YT);
   a.FT = (double*)(w + L.FT); a.U1 = (double*)(w + L.U1); a.U2 = (double*)(w + L.U2); a.HC = (double*)(w + L.HC);
-  a.G2 = (double*)(w + L.G2); a.LU = (double*)(w + L.LU); a.lu_stride = rr_lu_stride(m); a.lu_ldr = rr_lu_ldr(m); a.dinv = (double*)(w + L.dinv); a.pst = (int*)(w + L.pst);
+  a.G2 = (double*)(w + L.G2); a.JB = (double*)(w + L.JB); a.LU = (double*)(w + L.LU); a.lu_stride = rr_lu_stride(m); a.lu_ldr = rr_lu_ldr(m); a.dinv = (double*)(w + L.dinv); a.pst = (int*)(w + L.pst);
   a.hs = (double*)(w + L.hs); a.flg = (int*)(w + L.flg);
   int sms = 0;
   CK_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, m->device));
   const unsigned tb = 256, gn = (unsigned)((n + tb - 1) / tb);
   int* h_cnt = nullptr;  // pinned: the active count comes back once per round
-  CK_CUDA(cudaHostAlloc((void**)&h_cnt, 2 * sizeof(int), cudaHostAllocDefault));
+  CK_CUDA(cudaHostAlloc((void**)&h_cnt, 4 * sizeof(int), cudaHostAllocDefault));
   auto fail = [&](int32_t rc) { cudaFreeHost(h_cnt); return rc; };
+  long long nj = 0;   // reactors that need a fresh Jacobian in the coming round
   auto read_count = [&](long long* na) -> int32_t {
-    CK_CUDA(cudaMemcpyAsync(h_cnt, a.cnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK_CUDA(cudaMemcpyAsync(h_cnt, a.cnt, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
     CK_CUDA(cudaStreamSynchronize(st));
     *na = h_cnt[0];
+    nj = h_cnt[2];
     return CK_OK;
   };
   int32_t rc;
@@ -531,8 +573,10 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
     rhs_evals += 2 * (unsigned long long)na;
   }
   ros_guard_kernel<<<gn, tb, 0, st>>>(a);
+  ros_lists_kernel<<<(unsigned)((n + 1023) / 1024), 1024, 0, st>>>(a);
   ros_swap_kernel<<<1, 1, 0, st>>>(a);
   std::swap(a.act, a.act2);
+  std::swap(a.jl, a.jl2);
   if ((rc = read_count(&na))) return fail(rc);
   // the tail (few survivors: a round costs one thread-per-reactor wave whatever the count) goes to the fused kernel
   const long long tail = std::min<long long>(4096, std::max<long long>(n / 8, 1));
@@ -540,17 +584,22 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   while (na >= tail && na > 0) {
     const unsigned ga = (unsigned)((na + tb - 1) / tb);
     ros_gather_kernel<<<ga, tb, 0, st>>>(a, N);
-    rc = (jblock == 512) ? launch_jac_rows_rm<512>(m, a, na, sms, st) : launch_jac_rows_rm<224>(m, a, na, sms, st);
-    if (rc) return fail(rc);
+    if (nj > 0) {
+      rc = (jblock == 512) ? launch_jac_rows_rm<512>(m, a, nj, sms, st) : launch_jac_rows_rm<224>(m, a, nj, sms, st);
+      if (rc) return fail(rc);
+    }
     if ((rc = coop_dispatch(m, a, na, sms, 0, st))) return fail(rc);
     if ((rc = ck_rhs(m, na, a.YT, a.cap, a.Pw, a.FT, a.cap, st))) return fail(rc);
     if ((rc = coop_dispatch(m, a, na, sms, 1, st))) return fail(rc);
     if ((rc = ck_rhs(m, na, a.YT, a.cap, a.Pw, a.FT, a.cap, st))) return fail(rc);
     if ((rc = coop_dispatch(m, a, na, sms, 2, st))) return fail(rc);
+    ros_lists_kernel<<<(unsigned)((n + 1023) / 1024), 1024, 0, st>>>(a);
     ros_swap_kernel<<<1, 1, 0, st>>>(a);
     std::swap(a.act, a.act2);
-    rhs_evals += 3 * (unsigned long long)na; jac_evals += (unsigned long long)na;
-    count_tpr(na, jblock); count_tpr(na, 512); count_tpr(na, 512);
+    std::swap(a.jl, a.jl2);
+    rhs_evals += 2 * (unsigned long long)na + (unsigned long long)nj; jac_evals += (unsigned long long)nj;
+    if (nj > 0) count_tpr(nj, jblock);
+    count_tpr(na, 512); count_tpr(na, 512);
     slots_act += 3.0 * na * N; slots_tot += 3.0 * na * G;
     rounds++;
     if ((rc = read_count(&na))) return fail(rc);
@@ -623,7 +672,7 @@ extern "C" int32_t ck_jac_batched(const ck_mech* m, int64_t n, const double* y, 
   cudaStream_t st = (cudaStream_t)stream;
   const size_t N = m->K + 1;
   char* w = (char*)ws;
-  JacOut o;
+  JacOut o{};
   o.f = (double*)w; o.ldf = n; w += al256(N * (size_t)n * 8);
   o.hc = (double*)w; o.ldh = n; w += al256((size_t)jac_hc_rows(m->K) * n * 8);
   o.g2 = (double*)w; o.ldg = n;
