@@ -40,12 +40,13 @@ def _run(oracle, name, n, solver=None, jac_mode=0, flags=0, dt=None, flame=False
     return g, res, ref, mech
 
 
-def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
+def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False, pop=None):
     """fd: ROS4 with the finite-difference Jacobian.  Its columns carry rounding noise eps D / sigma_j (reading G12), which
     differs between any two correct executions and which the step controller amplifies: the two CPU builds of the oracle
     already differ by 2 accepted / 6 rejected attempts per reactor (tests/test_oracle_p3.py), so the count slack is 2
     (6 for rejected attempts) instead of 1, the batch total of rejected attempts may differ by 10 %, and states are
-    judged by DESIGN.md P3."""
+    judged by DESIGN.md P3.  pop: columns that are a RANDOM sample of the workload (P3's 99.9 % clause is a statement about
+    the population; reactors picked because they are the longest chains are judged by the exact-solution clause alone)."""
     slack = 2 if fd else 1
     st = res["status"].cpu().numpy()
     assert np.array_equal(st, ref["status"]) and np.all(st == 0)
@@ -56,7 +57,7 @@ def _check(g, res, ref, n_species, frac_count=0.05, tight=None, fd=False):
     if tight is None:
         assert not bad.any(), (int(bad.sum()), float(np.abs(Y - Yo).max()))
     else:  # DESIGN.md P3
-        assert bad.mean() <= 1e-3, float(bad.mean())
+        assert (bad if pop is None else bad[:, pop]).mean() <= 1e-3, float(bad.mean())
         print("P3 fallback:", int(bad.sum()), "of", bad.size, "entries in", len(np.unique(np.where(bad)[1])), "reactors")
         yt = tight(np.unique(np.where(bad)[1]))
         for r, col in yt.items():
@@ -148,6 +149,36 @@ def test_rkf45_c4_subset(oracle):
     assert 0.3 < rep["simt_efficiency"] <= 1.0
 
 
+@pytest.mark.parametrize("n", [100, 700])
+def test_rkf45_small_batches_skip_the_thread_per_reactor_phase(oracle, n):
+    """Below 16,384 reactors everything goes to the finishers after the 24-attempt classification pass (n <= #SMs: every
+    unfinished reactor on the wide kernel; more: stragglers wide, the others narrow)."""
+    g, res, ref, mech = _run(oracle, "C4", n)
+    rep = _check(g, res, ref, 53, tight=ref["tight"])
+    assert rep["rhs_evals"] == 6 * rep["attempts"] + 2 * n and rep["rounds"] >= 2
+
+
+def test_ros_rounds_jacobian_reuse_changes_no_result(oracle):
+    """flags bit 6: a fresh Jacobian for every attempt.  The default keeps J(y_n) across a rejected attempt; the values
+    are the same, so the two runs must agree bit for bit while the Jacobian count drops."""
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+    mech, y, p, cfg = make_config("C3", n=900)
+    M = ck.Mechanism(mech)
+    out = []
+    for flags in (8, 8 | 64):
+        yd = torch.from_numpy(y).cuda()
+        res = M.integrate("ros", yd, torch.from_numpy(p).cuda(), cfg["dt"], flags=flags)
+        out.append((yd.cpu().numpy(), res))
+    (ga, ra), (gb, rb) = out
+    assert np.array_equal(ga, gb)
+    for k in ("n_accept", "n_reject", "status"):
+        assert torch.equal(ra[k], rb[k])
+    assert ra["report"]["attempts"] == rb["report"]["attempts"] == rb["report"]["jac_evals"]
+    assert ra["report"]["rejected"] > 0 and ra["report"]["jac_evals"] < ra["report"]["attempts"]
+
+
 def test_rkf45_static_vs_refill(oracle):
     """The divergence-control layer changes scheduling only: same results, higher SIMT efficiency."""
     g1, r1, ref, _ = _run(oracle, "C4", 2048, flags=1)
@@ -226,8 +257,14 @@ def test_full_size_sampled(oracle, name, nsample):
     g = yd.cpu().numpy()
     assert np.isfinite(g).all() and int(res["report"]["n_failed"]) == 0
     assert np.all(np.abs(g[1:].sum(0) - 1.0) < 1e-6)               # property at any size
-    idx = np.unique(np.concatenate([np.arange(8), np.arange(n - 8, n),
-                                    np.random.default_rng(11).integers(0, n, nsample)]))
+    picks = [np.arange(8), np.arange(n - 8, n), np.random.default_rng(11).integers(0, n, nsample)]
+    if cfg["call"] == "rkf45":
+        # the divergence-control layer routes reactors by their step counts: make sure the sample holds the longest
+        # chains (wide finisher) and reactors of the middle class (narrow finisher), not only the bulk
+        order = np.argsort(-(res["n_accept"] + res["n_reject"]).cpu().numpy(), kind="stable")
+        picks += [order[:10], order[np.random.default_rng(12).integers(300, 12000, 24)]]
+    idx = np.unique(np.concatenate(picks))
+    pop = np.isin(idx, np.concatenate(picks[:3]))
     O = oracle.Mech(mech)
     ys = np.ascontiguousarray(y[:, idx]); ps = np.ascontiguousarray(p[idx])
     ref = O.integrate(cfg["call"], ys, ps, cfg["dt"], rtol=cfg["rtol"], atol=cfg["atol"], nthreads=16)
@@ -242,4 +279,4 @@ def test_full_size_sampled(oracle, name, nsample):
     st, na, nr = res["status"][ti], res["n_accept"][ti], res["n_reject"][ti]
     sub = dict(status=st, n_accept=na, n_reject=nr,
                report=dict(accepted=int(na.sum()), rejected=int(nr.sum()), attempts=int((na + nr).sum()), n_failed=0))
-    _check(g[:, idx], sub, ref, mech["n_species"], tight=tight if cfg["call"] == "rkf45" else None)
+    _check(g[:, idx], sub, ref, mech["n_species"], tight=tight if cfg["call"] == "rkf45" else None, pop=pop)
