@@ -568,12 +568,16 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
     // Touch every kernel of the flow BEFORE the first launch: CUDA loads kernels lazily, and a first-use load issued while
     // another kernel runs waits for it -- the side-by-side phases of the first call of a process would run one after
     // the other (measured: 3.4 s instead of 1.45 s for config 4).
+    // The shared-memory opt-ins are made here as well, so that nothing that can fail is left for the time when y is
+    // half-integrated.
     cudaFuncAttributes fa;
-    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_wide_kernel<WIDE_G>));
-    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<32>));
-    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<64>));
-    CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_coop_kernel<128>));
-    CK_CUDA(cudaFuncGetAttributes(&fa, rkf_order_kernel));
+    const size_t smem_w0 = rkf_wide_smem_doubles(m->K, m->R, m->dev.r_tb, m->dev.n_tent) * sizeof(double);
+    if (m->K <= 128 && smem_w0 <= 227 * 1024)
+      CK_CUDA(cudaFuncSetAttribute(rkf45_wide_kernel<WIDE_G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_w0));
+    CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+    CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+    CK_CUDA(cudaFuncSetAttribute(rkf45_coop_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+    CK_CUDA(cudaFuncSetAttribute(rkf_order_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RKF_ORDER_MAX * 12));
     CK_CUDA(cudaFuncGetAttributes(&fa, rkf_bucket_kernel));
     CK_CUDA(cudaFuncGetAttributes(&fa, rkf45_kernel<512, true>));
   }

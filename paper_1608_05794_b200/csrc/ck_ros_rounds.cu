@@ -579,7 +579,11 @@ int32_t ros_rounds_run(const ck_mech* m, int64_t n, double* y, int64_t ld, const
   std::swap(a.jl, a.jl2);
   if ((rc = read_count(&na))) return fail(rc);
   // the tail (few survivors: a round costs one thread-per-reactor wave whatever the count) goes to the fused kernel
-  const long long tail = std::min<long long>(4096, std::max<long long>(n / 8, 1));
+  // A round costs a fixed latency whatever the count (the thread-per-reactor Jacobian alone takes ~2 ms for N = 54, ~3.7 ms
+  // for N = 112), the fused kernel a cost per reactor and attempt that grows like N^2..3 (0.19 us for N = 54, 1.4 us for
+  // N = 112, measured): the break-even is ~16 k reactors for N = 54 and ~4 k for N = 112.
+  const double bq = 54.0 / (double)N;
+  const long long tail = std::max<long long>(1, std::min<long long>(n / 4, std::max<long long>(2048, (long long)(16384.0 * bq * bq))));
   int rounds = 0;
   while (na >= tail && na > 0) {
     const unsigned ga = (unsigned)((na + tb - 1) / tb);

@@ -158,6 +158,16 @@ def test_rkf45_small_batches_skip_the_thread_per_reactor_phase(oracle, n):
     assert rep["rhs_evals"] == 6 * rep["attempts"] + 2 * n and rep["rounds"] >= 2
 
 
+@pytest.mark.parametrize("flags", [0, 32])
+def test_rkf45_on_the_111_species_model(oracle, flags):
+    """The finishers on the largest model: 784 reactions exceed one reaction per thread of the wide kernel (every
+    reaction thread walks several rows), four species per lane of its species warp, and species rows of the transposed
+    stoichiometry too long for the register-resident gather; flags bit 5 puts the same reactors on the narrow kernel."""
+    g, res, ref, mech = _run(oracle, "C5", 160, solver="rkf45", dt=1e-7, flags=flags)
+    rep = _check(g, res, ref, 111, tight=ref["tight"])
+    assert rep["rhs_evals"] == 6 * rep["attempts"] + 2 * 160 and rep["rounds"] >= 2
+
+
 def test_ros_rounds_jacobian_reuse_changes_no_result(oracle):
     """flags bit 6: a fresh Jacobian for every attempt.  The default keeps J(y_n) across a rejected attempt; the values
     are the same, so the two runs must agree bit for bit while the Jacobian count drops."""
