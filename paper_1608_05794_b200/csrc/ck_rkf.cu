@@ -605,11 +605,11 @@ extern "C" int32_t ck_integrate_rkf45(const ck_mech* m, int64_t n, double* y, in
       const size_t smem_w = rkf_wide_smem_doubles(m->K, m->R, m->dev.r_tb, m->dev.n_tent) * sizeof(double);
       const bool wide_ok = m->K <= 128 && smem_w <= 227 * 1024 && !(o->flags & 32);
       // SM shares.  The three phases that follow run side by side, and the resumed thread-per-reactor kernel and the wide
-      // finisher each need a whole SM per CTA, so the split is made here: the stragglers get one SM each (at most 40 % of
-      // the machine), the rest is divided between the resumed kernel and the narrow finisher in proportion to their
+      // finisher each need a whole SM per CTA, so the split is made here: the stragglers get one SM each (at most 30 % of
+      // the machine: measured on config 4, 20 % makes their queue the long pole, 40 % starves the other two), the rest is divided between the resumed kernel and the narrow finisher in proportion to their
       // predicted work (measured cost per attempt: 2.1 us of an SM thread-per-reactor, 7.4 us on narrow CTAs); the narrow
       // finisher is launched with more CTAs than fit, so it also takes over every SM the other two give back.
-      const long long gW = std::min<long long>(nW, (nC + nM > 0) ? (2 * sms) / 5 : sms);
+      const long long gW = std::min<long long>(nW, (nC + nM > 0) ? (3 * sms) / 10 : sms);
       const double eb = 2.1 * (double)hs.sum_pred[0], em = 7.4 * (double)hs.sum_pred[1];
       const long long rem = sms - (wide_ok ? gW : 0);
       long long gC = rem;
