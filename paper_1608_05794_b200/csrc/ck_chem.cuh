@@ -220,7 +220,6 @@ template <int CS, bool WANT_AUX, int TYPE = -1>
 __device__ __forceinline__ double reaction_q(const MechDev& m, int r, const RxnConst& k, const TState& t,
                                              const double* __restrict__ C, double Ctot, RateAux* aux,
                                              const double* __restrict__ xrow = nullptr) {
-  const int R = m.R;
   const double beta = k.beta, Ta = k.Ta;
   const double c1 = k.c1, c2 = k.c2, c3 = k.c3, c4 = k.c4, c5 = k.c5, c6 = k.c6;
   const double T = t.T;

@@ -393,7 +393,6 @@ __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, lon
   const uint32_t wt = tbase + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * jac_npt(m.K));
   double* Cs = sm + tid;
   double* stage = sm + (size_t)(m.K + 1) * BLOCK;
-  const int N = m.K + 1;
   for (long long b = blockIdx.x; b * BLOCK < n; b += gridDim.x) {
     const long long r = b * BLOCK + tid;
     const bool act = r < n;

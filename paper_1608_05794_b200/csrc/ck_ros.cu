@@ -131,7 +131,6 @@ template <int G>
 __device__ __forceinline__ double estimate_h0_coop(const MechDev& m, RosShared& s, double p, double dt, double rtol,
                                                    double atol) {
   const int N = m.K + 1, tid = threadIdx.x;
-  TState t;
   rhs_stage<G>(&m, (int)(s.y - s.A), p, (int)(s.f0 - s.A));
   const double d0 = wrms_coop<G>(s.y, s.y, N, rtol, atol, s.c.red);
   const double d1 = wrms_coop<G>(s.f0, s.y, N, rtol, atol, s.c.red);
@@ -243,7 +242,6 @@ __global__ void __launch_bounds__(G, ros_min_ctas(G)) ros4_kernel(const __grid_c
       double* const Lb = s.c.dqs;
       double* const Ub = s.c.dqs + 3 * N;
       if constexpr (NS < 0) lu_compact4<G>(s.A, lda, N, pstep, Lb, Ub);
-      TState t;
       if constexpr (REG_FULL) solve_rows_smem<NS, G>(s.A, lda, pstep, s.f0, s.u1, s.c.red + 36);
       else if constexpr (NS < 0) {
         double bb = (tid < N) ? s.f0[tid] : 0.0;

@@ -237,6 +237,34 @@ def test_integrate_edge_cases(oracle):
     assert rc == 3
 
 
+@pytest.mark.parametrize("n,max_steps", [(120, 300), (600, 300), (600, 20)])
+def test_rkf45_step_limit_through_the_finishers(oracle, n, max_steps):
+    """max_steps exhausted inside the wide finisher (n <= #SMs: every unfinished reactor), inside the narrow one (larger
+    n: the middle class), and inside the classification pass itself (limit below its 24 attempts): status 1 for exactly
+    the reactors the oracle stops, the same attempt counts, and the last accepted state."""
+    import torch
+    import paper_1608_05794_b200 as ck
+    from synth_inputs import make_config
+    mech, y, p, cfg = make_config("C4", n=n)
+    M = ck.Mechanism(mech)
+    yd = torch.from_numpy(y).cuda()
+    r = M.integrate("rkf45", yd, torch.from_numpy(p).cuda(), cfg["dt"], max_steps=max_steps)
+    ref = oracle.Mech(mech).integrate("rkf45", y, p, cfg["dt"], max_steps=max_steps, nthreads=16)
+    st = r["status"].cpu().numpy()
+    att = (r["n_accept"] + r["n_reject"]).cpu().numpy()
+    att_ref = ref["n_accept"] + ref["n_reject"]
+    assert (st == 1).any() and set(np.unique(st)) <= {0, 1} and ((st == 0).any() or max_steps < 30)   # the quickest reactor takes ~30
+    # a reactor stops at the limit on both sides unless its attempt count sits within one flip of it (DESIGN.md P2)
+    clear = np.abs(att_ref - max_steps) > 1
+    assert np.array_equal(st[clear & (att_ref < max_steps)], ref["status"][clear & (att_ref < max_steps)])
+    assert np.all(att[st == 1] == max_steps) and np.all(att <= max_steps)
+    assert r["report"]["n_failed"] == int((st == 1).sum())
+    g = yd.cpu().numpy()
+    assert np.isfinite(g).all()
+    done = (st == 0) & (ref["status"] == 0)
+    assert np.all(np.abs(g[0, done] - ref["y"][0, done]) <= 1e-5 * ref["y"][0, done])
+
+
 def test_integrate_host_entry_point(oracle):
     import paper_1608_05794_b200 as ck
     from synth_inputs import make_config
