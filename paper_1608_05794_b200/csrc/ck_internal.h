@@ -76,6 +76,7 @@ int32_t cuda_fail(cudaError_t e, const char* what);
 
 struct ck_mech {
   int device = 0;
+  int sms = 148;              // SM count of `device` (grid sizing)
   ck::MechDev dev;            // device view
   void* arena = nullptr;      // device allocation backing `dev`
   size_t arena_bytes = 0;

@@ -304,6 +304,7 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   ck_mech* m = new ck_mech;
   m->device = device;
   cudaError_t e = cudaSetDevice(device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&m->sms, cudaDevAttrMultiProcessorCount, device);
   if (e == cudaSuccess) e = cudaMalloc(&m->arena, a.buf.size());
   if (e == cudaSuccess) e = cudaMemcpy(m->arena, a.buf.data(), a.buf.size(), cudaMemcpyHostToDevice);
   if (e != cudaSuccess) {
@@ -330,7 +331,6 @@ extern "C" int32_t ck_mech_load(const ck_mech_desc* d, int32_t device, ck_mech**
   v.tptr = (const int*)(base + otp); v.tent = (const int*)(base + ote); v.n_tent = (int)tent.size(); v.perm = (const int*)(base + operm);
   m->K = K; m->R = R; m->n_tb = cnt[1]; m->n_lind = cnt[2]; m->n_troe = cnt[3]; m->n_rev = n_rev;
   m->n_part = n_part; m->n_eff = (long long)espec.size();
-  if (getenv("CK_DEBUG")) fprintf(stderr, "ck_mech_load: K=%d R=%d groups: r_22=%d r_dup=%d r_tb=%d r_lind=%d r_troe=%d r_tbf=%d nT=%d\n", K, R, v.r_22, v.r_dup, v.r_tb, v.r_lind, v.r_troe, v.r_tbf, nT);
   *out = m;
   return CK_OK;
 }

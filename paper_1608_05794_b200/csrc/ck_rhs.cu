@@ -66,7 +66,7 @@ static int32_t launch_rhs_tmem(const ck_mech* m, long long n, const double* y, l
 int rhs_tmem_block(const ck_mech* m, long long n) {
   const int K = m->K, rs = m->dev.rstride;
   if (K + 1 <= 64) {
-    if (n >= 148 * 256 && rhs_tmem_smem_bytes(K, rs, 512) <= 227 * 1024) return 512;
+    if (n >= (long long)m->sms * 256 && rhs_tmem_smem_bytes(K, rs, 512) <= 227 * 1024) return 512;
     if (n >= 2048 && rhs_tmem_cols(K, 128) != 0) return 128;
     return 0;
   }
@@ -94,7 +94,7 @@ extern "C" int32_t ck_rhs(const ck_mech* m, int64_t n, const double* y, int64_t 
     case 128: return launch_rhs_tmem<128>(m, n, y, ld, p, dydt, ld_out, st);
     default: break;
   }
-  switch (rhs_pick_block(m->K, m->dev.rstride, n)) {
+  switch (rhs_pick_block(m->K, m->dev.rstride, n, m->sms)) {
     case 256: return launch_rhs<256>(m, n, y, ld, p, dydt, ld_out, st);
     case 128: return launch_rhs<128>(m, n, y, ld, p, dydt, ld_out, st);
     case 64: return launch_rhs<64>(m, n, y, ld, p, dydt, ld_out, st);
@@ -111,6 +111,6 @@ extern "C" int32_t ck_rhs_variant(const ck_mech* m, int64_t n, int32_t* block, i
   if (!m || !block || !tmem) { set_error("ck_rhs_variant: null argument"); return CK_EINVAL; }
   const int b = ck::rhs_tmem_block(m, n);
   *tmem = b != 0;
-  *block = b ? b : rhs_pick_block(m->K, m->dev.rstride, n);
+  *block = b ? b : rhs_pick_block(m->K, m->dev.rstride, n, m->sms);
   return CK_OK;
 }

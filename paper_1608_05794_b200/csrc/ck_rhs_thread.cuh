@@ -153,12 +153,12 @@ __device__ __forceinline__ void rhs_thread(const MechDev& m, const double* __res
 }
 
 // largest block whose columns fit in shared memory, halved while the grid would leave most SMs idle
-inline int rhs_pick_block(int K, int rstride, long long n) {
+inline int rhs_pick_block(int K, int rstride, long long n, int sms) {
   const size_t cap = 227 * 1024;
   int block = 256;
   while (block >= 32 && rhs_smem_bytes(K, rstride, block) > cap) block >>= 1;
   if (block < 32) return 0;
-  while (block > 32 && (n + block - 1) / block < 148) block >>= 1;
+  while (block > 32 && (n + block - 1) / block < sms) block >>= 1;
   return block;
 }
 

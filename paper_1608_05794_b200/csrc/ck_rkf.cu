@@ -461,11 +461,11 @@ cudaError_t plan_for(const ck_mech* m, long long n, RkfPlan* pl) {
 
 int32_t rkf_plan(const ck_mech* m, long long n, RkfPlan* pl) {
   CK_CUDA(cudaSetDevice(m->device));
-  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= 148 * 256) {
+  if (m->K + 1 <= 64 && rhs_tmem_smem_bytes(m->K, m->dev.rstride, 512) <= 227 * 1024 && n >= (long long)m->sms * 256) {
     CK_CUDA((plan_for<512, true>(m, n, pl)));
     return CK_OK;
   }
-  const int block = rhs_pick_block(m->K, m->dev.rstride, n);
+  const int block = rhs_pick_block(m->K, m->dev.rstride, n, m->sms);
   switch (block) {
     case 256: CK_CUDA((plan_for<256, false>(m, n, pl))); break;
     case 128: CK_CUDA((plan_for<128, false>(m, n, pl))); break;

@@ -45,7 +45,9 @@ int32_t waste_launch(int64_t n, const int32_t* n_accept, const int32_t* n_reject
   if (n == 0) return CK_OK;
   if (!n_accept || !W) { set_error("%s: null pointer", who); return CK_EINVAL; }
   const long long units = (n + (long long)P * m - 1) / ((long long)P * m);
-  const long long blocks = std::max<long long>(1, std::min<long long>((units + 7) / 8, 148 * 8));
+  int dev = 0, sms = 148;   // no mechanism handle here: ask the current device
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const long long blocks = std::max<long long>(1, std::min<long long>((units + 7) / 8, (long long)sms * 8));
   waste_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(n, n_accept, n_reject, P, m, W);
   CK_CUDA(cudaGetLastError());
   return CK_OK;
