@@ -129,7 +129,7 @@ __device__ __forceinline__ void jac_phaseA_row(const MechDev& m, int r, const do
 template <int BLOCK, bool RM>
 __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* __restrict__ yin, long long ldin, double p,
                                                 const JacOut& o, long long slot, long long gslot, double* __restrict__ Cs, uint32_t wt,
-                                                double* __restrict__ stage, bool store) {
+                                                double* __restrict__ stage, bool store, int part = 0, int nsub = 1) {
   const int K = m.K, R = m.R, rs = m.rstride, N = K + 1;
   const int tid = threadIdx.x;
   const TState t = make_tstate(m, yin[0]);
@@ -233,7 +233,9 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
   double sfc = 0.0;  // sum_k f_k cc_k
   constexpr int CB = BLOCK * 8;  // bytes between C columns
   const char* Cb = reinterpret_cast<const char*>(Cs);
-  for (int k = 0; k < K; ++k) {
+  // nsub > 1: this thread is one of nsub that work on the SAME reactor (each ran phase A in full, on its own columns and
+  // scratch, and wrote the same f / hc values); the species rows are dealt out round-robin
+  for (int k = part; k < K; k += nsub) {
     double sig = 0.0, tht = 0.0, dns = 0.0;
     const int e0 = tb.tptr[k], e1 = tb.tptr[k + 1];
     // software pipeline: the scratch values of entry e + 1 are in flight while entry e is processed
@@ -368,7 +370,12 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
     if (store && odd_row) rowbase[NP - 1] = carry;
     tm_wait_st();
   }
-  if (store) hc[(size_t)(2 * K) * o.ldh] = -sfc - fT * dcp * icps;
+  if (nsub > 1) {   // the sum runs over ALL rows: redo it from this thread's own phase-A outputs
+    sfc = 0.0;
+    if (store && part == 0)
+      for (int k = 0; k < K; ++k) sfc = fma(fout[(size_t)(1 + k) * o.ldf], hc[(size_t)(K + k) * o.ldh], sfc);
+  }
+  if (store && part == 0) hc[(size_t)(2 * K) * o.ldh] = -sfc - fT * dcp * icps;
 }
 
 // One CTA per SM, persistent over batches of BLOCK slots (as rhs_kernel_tmem).  n_dev (optional) overrides n with a
@@ -376,7 +383,7 @@ __device__ __forceinline__ void jac_thread_tmem(const MechDev& m, const double* 
 template <int BLOCK, bool RM>
 __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, long long n, const int* __restrict__ n_dev,
                                                             const double* __restrict__ y, long long ld,
-                                                            const double* __restrict__ p, JacOut o) {
+                                                            const double* __restrict__ p, JacOut o, const int nsub = 1) {
   extern __shared__ double sm[];
   __shared__ uint32_t s_tmem;
   if (n_dev) n = *n_dev;
@@ -393,15 +400,22 @@ __global__ void __launch_bounds__(BLOCK, 1) jac_rows_kernel(const MechDev m, lon
   const uint32_t wt = tbase + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * 2 * jac_npt(m.K));
   double* Cs = sm + tid;
   double* stage = sm + (size_t)(m.K + 1) * BLOCK;
-  for (long long b = blockIdx.x; b * BLOCK < n; b += gridDim.x) {
-    const long long r = b * BLOCK + tid;
+  // nsub threads per reactor (the caller picks nsub > 1 when the batch leaves lanes idle: the kernel's duration is one
+  // thread's latency, most of it the K species rows, whatever the count).  The parts are dealt out by WARP (threads
+  // [g BLOCK / nsub, (g + 1) BLOCK / nsub) take part g): the tensor-memory accesses are warp-collective, so the lanes of a
+  // warp must walk the same rows.  nsub must divide BLOCK / 32.
+  const int per = BLOCK / nsub;                 // reactors per CTA pass
+  const int part = tid / per, local = tid - part * per;
+  for (long long b = blockIdx.x; b * per < n; b += gridDim.x) {
+    const long long r = b * per + local;
     const bool act = r < n;
     const long long rr = act ? r : n - 1;
+    const long long gs = (long long)part * n + rr;   // scratch column of this thread: dense per part, < nsub * n
     const long long col = o.list ? (long long)o.list[rr] : rr;   // which column of y / p / f / hc / J this thread works on
     JacOut oo = o;
     if (RM) oo.J = o.J + (size_t)col * o.sstride;
     else oo.J = o.J + col;
-    jac_thread_tmem<BLOCK, RM>(m, y + col, ld, p[col], oo, col, rr, Cs, wt, stage, act);
+    jac_thread_tmem<BLOCK, RM>(m, y + col, ld, p[col], oo, col, gs, Cs, wt, stage, act, part, nsub);
   }
   asm volatile("tcgen05.fence::before_thread_sync;");
   __syncthreads();

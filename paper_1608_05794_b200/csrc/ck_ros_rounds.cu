@@ -479,8 +479,14 @@ int32_t launch_jac_rows_rm(const ck_mech* m, const RoundArgs& a, long long na, i
   o.f = a.F0; o.ldf = a.cap; o.J = a.JB; o.ldJ = 0; o.ldr = a.lu_ldr; o.sstride = a.lu_stride;
   o.hc = a.HC; o.ldh = a.cap; o.g2 = a.G2; o.ldg = a.cap;
   o.list = a.jl;   // thread i works on reactor jl[i]: state straight from y, outputs by reactor
-  const long long grid = std::max<long long>(1, std::min<long long>((na + BLOCK - 1) / BLOCK, sms));
-  jac_rows_kernel<BLOCK, true><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, na, a.cnt + 2, a.y, a.ld, a.p, o);
+  // several threads per reactor while the list leaves lanes (and scratch columns) idle; nsub divides BLOCK / 32
+  int nsub = 1;
+  const long long lanes = std::min<long long>((long long)sms * BLOCK, a.cap);   // a.cap: columns of the scratch array
+  if (BLOCK == 512) { while (nsub < 8 && na * nsub * 2 <= lanes) nsub *= 2; }
+  else if (BLOCK == 224 && na * 7 <= lanes) nsub = 7;
+  const long long per = BLOCK / nsub;
+  const long long grid = std::max<long long>(1, std::min<long long>((na + per - 1) / per, sms));
+  jac_rows_kernel<BLOCK, true><<<(unsigned)grid, BLOCK, smem, st>>>(m->dev, na, a.cnt + 2, a.y, a.ld, a.p, o, nsub);
   CK_CUDA(cudaGetLastError());
   return CK_OK;
 }
